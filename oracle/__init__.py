@@ -1,0 +1,251 @@
+"""ctypes front-end of the CPU oracle (oracle/bonsai_oracle.cpp).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this package.  It imports nothing from paper_1204_2280_b200 (inputs are passed in).
+Each function is a thin marshalling layer over the C++ routine of the same name; see that
+file for the passage of the paper / the DESIGN.md reading each one follows.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass, field
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.oracle_tree.restype = C.c_uint32
+        _lib.oracle_groups.restype = C.c_uint32
+    return _lib
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a
+
+
+def box(pos_mass):
+    pm = _f32(pos_mass)
+    lo = np.zeros(3, np.float32)
+    side = C.c_double(0)
+    lib().oracle_box(_p(pm, C.c_float), C.c_uint32(pm.shape[0]), _p(lo, C.c_float), C.byref(side))
+    return lo, side.value
+
+
+def keys(pos_mass, lo, side):
+    pm = _f32(pos_mass)
+    lo = _f32(lo)
+    out = np.zeros((pm.shape[0], 3), np.uint32)
+    lib().oracle_keys(_p(pm, C.c_float), C.c_uint32(pm.shape[0]), _p(lo, C.c_float), C.c_double(side),
+                      _p(out, C.c_uint32))
+    return out
+
+
+def decode_key(key):
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    q = np.zeros(3, np.uint32)
+    lib().oracle_decode_key(_p(k, C.c_uint32), _p(q, C.c_uint32))
+    return q
+
+
+def sort(keys_):
+    k = np.ascontiguousarray(keys_, dtype=np.uint32)
+    perm = np.zeros(k.shape[0], np.uint32)
+    lib().oracle_sort(_p(k, C.c_uint32), C.c_uint32(k.shape[0]), _p(perm, C.c_uint32))
+    return perm
+
+
+def reorder(pos_mass, keys_, perm):
+    pm = _f32(pos_mass)
+    k = np.ascontiguousarray(keys_, dtype=np.uint32)
+    spm = np.zeros_like(pm)
+    sk = np.zeros_like(k)
+    lib().oracle_reorder(_p(pm, C.c_float), _p(k, C.c_uint32), _p(perm, C.c_uint32), C.c_uint32(pm.shape[0]),
+                         _p(spm, C.c_float), _p(sk, C.c_uint32))
+    return spm, sk
+
+
+@dataclass
+class Tree:
+    n_cells: int
+    level: np.ndarray
+    first: np.ndarray
+    count: np.ndarray
+    first_child: np.ndarray
+    n_child: np.ndarray
+    parent: np.ndarray
+    level_offsets: np.ndarray
+    com_m: np.ndarray = None
+    quad: np.ndarray = None
+    delta: np.ndarray = None
+    lside: np.ndarray = None
+
+
+def tree(sorted_keys, nleaf=16, cap_cells=None):
+    sk = np.ascontiguousarray(sorted_keys, dtype=np.uint32)
+    n = sk.shape[0]
+    cap = cap_cells if cap_cells is not None else max(4096, 2 * n + 64)
+    arrs = [np.zeros(cap, np.uint32) for _ in range(6)]
+    lo = np.zeros(32, np.uint32)
+    nc = lib().oracle_tree(_p(sk, C.c_uint32), C.c_uint32(n), C.c_uint32(nleaf), C.c_uint32(cap),
+                           *[_p(a, C.c_uint32) for a in arrs], _p(lo, C.c_uint32))
+    if nc == 0xFFFFFFFF:
+        raise OverflowError("oracle_tree: more than cap_cells cells")
+    level, first, count, first_child, n_child, parent = [a[:nc].copy() for a in arrs]
+    return Tree(nc, level, first, count, first_child, n_child, parent, lo)
+
+
+@dataclass
+class Groups:
+    n_groups: int
+    n_active: int
+    active_list: np.ndarray
+    first: np.ndarray
+    count: np.ndarray
+    bmin: np.ndarray
+    bmax: np.ndarray
+
+
+def groups(mode, ncrit, sorted_pos_mass, t: Tree, active_sorted=None):
+    spm = _f32(sorted_pos_mass)
+    n = spm.shape[0]
+    act = None if active_sorted is None else np.ascontiguousarray(active_sorted, dtype=np.uint8)
+    active_list = np.zeros(n, np.uint32)
+    gfirst = np.zeros(n, np.uint32)
+    gcount = np.zeros(n, np.uint32)
+    bmin = np.zeros((n, 3), np.float32)
+    bmax = np.zeros((n, 3), np.float32)
+    na = C.c_uint32(0)
+    ng = lib().oracle_groups(C.c_uint32(mode), C.c_uint32(ncrit), C.c_uint32(n), _p(spm, C.c_float),
+                             C.c_uint32(t.n_cells), _p(t.first, C.c_uint32), _p(t.count, C.c_uint32),
+                             _p(t.first_child, C.c_uint32), _p(t.n_child, C.c_uint32),
+                             _p(act, C.c_uint8), _p(active_list, C.c_uint32), C.byref(na),
+                             _p(gfirst, C.c_uint32), _p(gcount, C.c_uint32), _p(bmin, C.c_float),
+                             _p(bmax, C.c_float))
+    return Groups(ng, na.value, active_list[:na.value].copy(), gfirst[:ng].copy(), gcount[:ng].copy(),
+                  bmin[:ng].copy(), bmax[:ng].copy())
+
+
+def multipoles(sorted_pos_mass, sorted_keys, lo, side, t: Tree):
+    spm = _f32(sorted_pos_mass)
+    sk = np.ascontiguousarray(sorted_keys, dtype=np.uint32)
+    lo = _f32(lo)
+    nc = t.n_cells
+    t.com_m = np.zeros((nc, 4), np.float32)
+    t.quad = np.zeros((nc, 6), np.float32)
+    t.delta = np.zeros(nc, np.float32)
+    t.lside = np.zeros(nc, np.float32)
+    lib().oracle_multipoles(_p(spm, C.c_float), _p(sk, C.c_uint32), C.c_uint32(spm.shape[0]),
+                            _p(lo, C.c_float), C.c_double(side), C.c_uint32(nc), _p(t.level, C.c_uint32),
+                            _p(t.first, C.c_uint32), _p(t.count, C.c_uint32), _p(t.com_m, C.c_float),
+                            _p(t.quad, C.c_float), _p(t.delta, C.c_float), _p(t.lside, C.c_float))
+    return t
+
+
+@dataclass
+class WalkResult:
+    acc: np.ndarray          # float64[n, 3], SORTED index; rows of particles not walked are NaN
+    pot: np.ndarray          # float64[n]
+    n_pp: np.ndarray         # uint32[n]
+    n_pc: np.ndarray         # uint32[n]
+    g_ntests: np.ndarray     # uint32[n_sel]
+    g_borderline: np.ndarray  # uint8[n_sel]
+    sel: np.ndarray = field(default=None)
+
+
+def walk(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel=None):
+    spm = _f32(sorted_pos_mass)
+    n = spm.shape[0]
+    sel_arr = None if sel is None else np.ascontiguousarray(sel, dtype=np.uint32)
+    n_sel = g.n_groups if sel_arr is None else sel_arr.shape[0]
+    acc = np.full((n, 3), np.nan, np.float64)
+    pot = np.full(n, np.nan, np.float64)
+    n_pp = np.zeros(n, np.uint32)
+    n_pc = np.zeros(n, np.uint32)
+    nt = np.zeros(max(n_sel, 1), np.uint32)
+    bl = np.zeros(max(n_sel, 1), np.uint8)
+    lib().oracle_walk(C.c_float(theta), C.c_float(eps), _p(spm, C.c_float), C.c_uint32(n),
+                      _p(t.first, C.c_uint32), _p(t.count, C.c_uint32), _p(t.first_child, C.c_uint32),
+                      _p(t.n_child, C.c_uint32), _p(t.com_m, C.c_float), _p(t.quad, C.c_float),
+                      _p(t.delta, C.c_float), _p(t.lside, C.c_float), _p(g.active_list, C.c_uint32),
+                      _p(g.first, C.c_uint32), _p(g.count, C.c_uint32), _p(g.bmin, C.c_float),
+                      _p(g.bmax, C.c_float), C.c_uint32(n_sel), _p(sel_arr, C.c_uint32),
+                      _p(acc, C.c_double), _p(pot, C.c_double), _p(n_pp, C.c_uint32), _p(n_pc, C.c_uint32),
+                      _p(nt, C.c_uint32), _p(bl, C.c_uint8))
+    return WalkResult(acc, pot, n_pp, n_pc, nt[:n_sel], bl[:n_sel], sel_arr)
+
+
+def walk_lists(theta, t: Tree, bmin, bmax, cap=None):
+    cap = cap if cap is not None else t.n_cells
+    pc = np.zeros(cap, np.uint32)
+    pp = np.zeros(cap, np.uint32)
+    npc, npp = C.c_uint32(0), C.c_uint32(0)
+    bmin = _f32(bmin)
+    bmax = _f32(bmax)
+    lib().oracle_walk_lists(C.c_float(theta), _p(t.first_child, C.c_uint32), _p(t.n_child, C.c_uint32),
+                            _p(t.com_m, C.c_float), _p(t.delta, C.c_float), _p(t.lside, C.c_float),
+                            _p(bmin, C.c_float), _p(bmax, C.c_float), C.c_uint32(cap),
+                            _p(pc, C.c_uint32), C.byref(npc), _p(pp, C.c_uint32), C.byref(npp))
+    return pc[:npc.value].copy(), pp[:npp.value].copy()
+
+
+def direct(pos_mass, eps, sinks=None):
+    pm = _f32(pos_mass)
+    n = pm.shape[0]
+    s = None if sinks is None else np.ascontiguousarray(sinks, dtype=np.uint32)
+    ns = n if s is None else s.shape[0]
+    acc = np.zeros((ns, 3), np.float64)
+    pot = np.zeros(ns, np.float64)
+    lib().oracle_direct(_p(pm, C.c_float), C.c_uint32(n), C.c_float(eps), C.c_uint32(ns),
+                        _p(s, C.c_uint32), _p(acc, C.c_double), _p(pot, C.c_double))
+    return acc, pot
+
+
+@dataclass
+class Step:
+    """Everything one force step produces, stage by stage (sorted order unless noted)."""
+    lo: np.ndarray
+    side: float
+    keys: np.ndarray            # load order
+    perm: np.ndarray
+    sorted_pos_mass: np.ndarray
+    sorted_keys: np.ndarray
+    tree: Tree
+    groups: Groups
+    walk: WalkResult = None
+
+    def to_load_order(self, a_sorted):
+        out = np.empty_like(a_sorted)
+        out[self.perm] = a_sorted
+        return out
+
+
+def build(pos_mass, nleaf=16, ncrit=64, group_mode=1, active_mask=None, cap_cells=None) -> Step:
+    """O1..O6: box, keys, sort, reorder, tree, groups, multipoles.  active_mask is in LOAD order."""
+    pm = _f32(pos_mass)
+    lo, side = box(pm)
+    k = keys(pm, lo, side)
+    perm = sort(k)
+    spm, sk = reorder(pm, k, perm)
+    t = tree(sk, nleaf, cap_cells)
+    act_sorted = None if active_mask is None else np.ascontiguousarray(active_mask, np.uint8)[perm]
+    g = groups(group_mode, ncrit, spm, t, act_sorted)
+    multipoles(spm, sk, lo, side, t)
+    return Step(lo, side, k, perm, spm, sk, t, g)
+
+
+def full_step(pos_mass, theta, eps, nleaf=16, ncrit=64, group_mode=1, active_mask=None, sel=None) -> Step:
+    s = build(pos_mass, nleaf, ncrit, group_mode, active_mask)
+    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
+    return s
