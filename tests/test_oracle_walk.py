@@ -22,15 +22,15 @@ def _numpy_direct(pm, eps, sinks):
     acc = np.zeros((len(sinks), 3))
     pot = np.zeros(len(sinks))
     for k, i in enumerate(sinks):
-      with np.errstate(divide="ignore"):
         d = x - x[i]
-          r2 = (d * d).sum(axis=1) + float(eps) ** 2
-          w = m / r2 ** 1.5
-          w[i] = 0.0
-          p = m / np.sqrt(r2)
-          p[i] = 0.0
-          acc[k] = (w[:, None] * d).sum(axis=0)
-          pot[k] = -p.sum()
+        r2 = (d * d).sum(axis=1) + float(eps) ** 2
+        r2[i] = 1.0  # self term: weight set to zero below
+        w = m / r2 ** 1.5
+        w[i] = 0.0
+        p = m / np.sqrt(r2)
+        p[i] = 0.0
+        acc[k] = (w[:, None] * d).sum(axis=0)
+        pot[k] = -p.sum()
     return acc, pot
 
 
