@@ -1,0 +1,169 @@
+/* =====================================================================================
+ * libbonsai -- C-ABI boundary of the B200-native Barnes-Hut force step.
+ *
+ * Method: "Bonsai: A GPU Tree-Code" (arXiv 1204.2280), cited as P:Lnn = line nn of the
+ * paper text.  The five timed sections of the paper (Results: "Sorting of
+ * the particles along a Space Filling Curve", "reordering of the particle properties
+ * ('moving')", "construction of the tree-datastructure", "computation of the multipole
+ * moments", "tree-traverse") map onto the calls below.  "All parts of the algorithm are
+ * executed on the GPU" (Abstract): every pointer documented "device" below is a
+ * CUDA device pointer, the host only sequences stages, and no call copies particle data
+ * between host and device.  The paper states no formula or constant; the exact
+ * arithmetic of every stage is the set of readings R1..R21 in DESIGN.md.
+ *
+ * Conventions
+ *   - All calls return an int: 0 (BONSAI_OK) or a negative BONSAI_E* code.  No exceptions, no
+ *     aborts, no output on stdout/stderr.
+ *   - All work is enqueued on the CUDA stream passed to bonsai_create() and the calls return
+ *     without waiting for it, except bonsai_sync() and bonsai_get_stage_ms().
+ *   - Memory: the CALLER owns every buffer (particles, masks, outputs and the workspace); the
+ *     library never allocates device memory.  The workspace must stay alive and untouched
+ *     between bonsai_create() and bonsai_destroy().  Device pointers handed out by the
+ *     bonsai_get_* calls point into the workspace and are valid until the next
+ *     bonsai_build_tree()/bonsai_walk() that rewrites them, or bonsai_destroy().
+ *   - "sorted order" = Morton order produced by bonsai_build_tree(); "load order" = the order of
+ *     the array given to bonsai_load().
+ * ===================================================================================== */
+#ifndef BONSAI_H_
+#define BONSAI_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BONSAI_OK          0
+#define BONSAI_EINVAL     (-1)  /* null / misaligned pointer, n = 0, n > n_max, bad parameter, NaN        */
+#define BONSAI_ESTATE     (-2)  /* call out of order (e.g. walk before multipoles)                        */
+#define BONSAI_ECAPACITY  (-3)  /* more cells than cap_cells, or traversal stack overflow (sticky, device) */
+#define BONSAI_ECUDA      (-4)  /* a CUDA runtime call failed                                             */
+#define BONSAI_ENOMEM     (-5)  /* workspace smaller than bonsai_workspace_bytes()                        */
+
+#define BONSAI_MAX_LEVEL   30   /* R1: 30 bits per axis, 90-bit Morton key (BASELINE.json north_star)     */
+#define BONSAI_N_STAGES    8
+
+typedef struct bonsai_ctx bonsai_ctx; /* opaque, host memory, owned by the library */
+
+/* Tunables.  A zeroed field takes the default in brackets. */
+typedef struct {
+    uint32_t nleaf;      /* [16] a cell with <= nleaf particles is a leaf (R7); 1..64                        */
+    uint32_t ncrit;      /* [64] maximum particles per walk group (R13); 1..64                               */
+    uint32_t group_mode; /* 0 = tree-cell groups, 1 = consecutive sorted chunks [1] (R13).  NOTE: because 0 is
+                            a legal value, group_mode is only defaulted when params == NULL.                   */
+    uint32_t cap_cells;  /* [n_max + 64] capacity of the cell arrays                                         */
+} bonsai_params;
+
+/* Bytes of device workspace bonsai_create() needs for up to n_max particles (0 on bad arguments). */
+size_t bonsai_workspace_bytes(uint32_t n_max, const bonsai_params* params);
+
+/* Create a context for up to n_max particles.
+ *   params         host pointer or NULL (all defaults, group_mode = 1)
+ *   workspace_dev  device pointer, 256-byte aligned, >= bonsai_workspace_bytes() bytes, caller-owned
+ *   cuda_stream    a cudaStream_t (NULL = the legacy default stream)
+ *   out            host pointer receiving the context
+ * Zero-fills the control block of the workspace on the stream.  EINVAL / ENOMEM / ECUDA. */
+int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_dev, size_t workspace_bytes,
+                  void* cuda_stream, bonsai_ctx** out);
+
+/* Hand the particles of this step to the library (particle arrays live on the device).
+ *   pos_mass_dev   device, float4[n] = (x, y, z, m), 16-byte aligned, load order.  NOT copied: it is read by
+ *                  bonsai_build_tree() (bounding box, keys, reorder) and must stay valid and unchanged until
+ *                  that call has completed on the stream.  Finite positions and m >= 0 are preconditions.
+ *   n              1 .. n_max
+ * Invalidates tree, multipoles and walk results.  EINVAL. */
+int bonsai_load(bonsai_ctx* ctx, const float* pos_mass_dev, uint32_t n);
+
+/* Stages a0..a4' ("sorting", "moving", "construction of the tree-datastructure"):
+ *   bounding box -> root cube (R3); 90-bit Morton keys (R1, R2, R4); stable radix sort of (key, index) (R5);
+ *   reorder of pos_mass into sorted order; octree over the sorted keys (R7: leaf <=> count <= nleaf or level 30,
+ *   sparse, chains kept, breadth-first numbering); walk groups over all particles with exact fp32 boxes (R13).
+ * ESTATE if nothing is loaded.  A cell overflow sets the sticky ECAPACITY flag reported by bonsai_sync(). */
+int bonsai_build_tree(bonsai_ctx* ctx);
+
+/* Stage a5 ("computation of the tree-properties (multipole moments)"): per cell the mass, centre
+ * of mass, the 6 raw second moments about the centre of mass (xx, yy, zz, xy, xz, yz), delta = |COM - geometric
+ * centre| and the cell side l (R8).  Accumulated in fp64, stored rounded once to fp32.  ESTATE before build. */
+int bonsai_compute_multipoles(bonsai_ctx* ctx);
+
+/* Stage a6 / a7 ("tree-traverse"): for every group, traverse from the root with the opening
+ * criterion  d2 > (l / theta + delta)^2  evaluated in fp32 exactly as R9 orders it (d = distance from the group's
+ * box to the cell's COM); accepted cells act on every particle of the group as monopole + quadrupole
+ * (particle-cell), rejected leaves particle by particle, with Plummer softening eps in every power of r (R10).
+ *   theta >= 0 (0 = open everything = direct summation through the tree), eps >= 0, both finite
+ *   active_mask_dev  device u8[n] in LOAD order, or NULL = all particles are sinks.  A non-NULL mask rebuilds
+ *                    the group list over the active particles for this call (R13, R19); all particles stay
+ *                    sources.  Must stay valid until the call completed on the stream.
+ *   acc_pot_dev_out  device float4[n] = (ax, ay, az, phi), load order, 16-byte aligned.  G = 1; phi is the
+ *                    potential per unit mass with the self term excluded (R11, R12).  Only entries of active
+ *                    particles are written.
+ * Per-particle interaction counts are kept for bonsai_get_counts().  EINVAL, ESTATE before multipoles. */
+int bonsai_walk(bonsai_ctx* ctx, float theta, float eps, const uint8_t* active_mask_dev, float* acc_pot_dev_out);
+
+/* Release the context (host memory only; the workspace belongs to the caller).  NULL is allowed. */
+void bonsai_destroy(bonsai_ctx* ctx);
+
+/* Wait for the stream and return the sticky device status (OK / ECAPACITY) or ECUDA. */
+int bonsai_sync(bonsai_ctx* ctx);
+
+/* ---- introspection (parity tests and reporting).  All pointers returned are DEVICE pointers. ---- */
+
+/* Root cube on the device: float[4] = (lo_x, lo_y, lo_z, side) (R3; side is a power of two). */
+int bonsai_get_box(bonsai_ctx* ctx, const float** box4_dev);
+
+/* Sorted keys, one u32 array per 30-bit word: hi = levels 1-10, mid = 11-20, lo = 21-30 (R1). */
+int bonsai_get_keys(bonsai_ctx* ctx, const uint32_t** hi_dev, const uint32_t** mid_dev, const uint32_t** lo_dev);
+
+/* perm[i] = load index of the i-th sorted particle; sorted pos_mass float4[n]. */
+int bonsai_get_perm(bonsai_ctx* ctx, const uint32_t** perm_dev);
+int bonsai_get_sorted_pos(bonsai_ctx* ctx, const float** pos_mass_dev);
+
+typedef struct {
+    uint32_t cap_cells;
+    const uint32_t* n_cells;       /* device u32[1]                                                     */
+    const uint32_t* level_offsets; /* device u32[32]: first cell of level L, [31] = n_cells             */
+    const uint32_t* level;         /* device u32[cap] each, structure of arrays (R7)                    */
+    const uint32_t* first;         /*   first sorted particle                                           */
+    const uint32_t* count;         /*   number of particles                                             */
+    const uint32_t* first_child;   /*   0 for a leaf                                                    */
+    const uint32_t* n_child;       /*   0 for a leaf                                                    */
+    const uint32_t* parent;        /*   0xFFFFFFFF for the root                                         */
+    const float* com_m;            /* device float4[cap]: COM x, y, z, mass (after multipoles)          */
+    const float* quad;             /* device float[6*cap]: xx, yy, zz, xy, xz, yz                       */
+    const float* delta;            /* device float[cap]                                                 */
+    const float* lside;            /* device float[cap]                                                 */
+} bonsai_cells_view;
+int bonsai_get_cells(bonsai_ctx* ctx, bonsai_cells_view* out);
+
+typedef struct {
+    const uint32_t* n_groups;    /* device u32[1]                                                       */
+    const uint32_t* n_active;    /* device u32[1]                                                       */
+    const uint32_t* active_list; /* device u32[n_active]: sorted index of the k-th active particle      */
+    const uint32_t* first;       /* device u32[n_groups]: offset into active_list                       */
+    const uint32_t* count;       /* device u32[n_groups]                                                */
+    const float* bmin;           /* device float[3*n_groups]                                            */
+    const float* bmax;           /* device float[3*n_groups]                                            */
+} bonsai_groups_view;
+/* The group list of the last bonsai_build_tree() (all active) or of the last masked bonsai_walk(). */
+int bonsai_get_groups(bonsai_ctx* ctx, bonsai_groups_view* out);
+
+/* Interaction counts of the last walk, per particle in LOAD order (R21): n_pp = particles in the opened
+ * leaves of the particle's group minus itself, n_pc = accepted cells of its group. */
+int bonsai_get_counts(bonsai_ctx* ctx, const uint32_t** n_pp_dev, const uint32_t** n_pc_dev);
+
+/* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events between stages from then on;
+ * bonsai_get_stage_ms() waits for the stream and writes milliseconds of the most recent execution of each
+ * stage: 0 bbox, 1 keys, 2 sort, 3 reorder, 4 build, 5 groups, 6 multipoles, 7 walk. */
+int bonsai_set_timing(bonsai_ctx* ctx, int enable);
+int bonsai_get_stage_ms(bonsai_ctx* ctx, float out_ms[BONSAI_N_STAGES]);
+
+/* Number of kernel launches the library has enqueued since bonsai_create(). */
+uint64_t bonsai_get_launch_count(bonsai_ctx* ctx);
+
+const char* bonsai_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BONSAI_H_ */

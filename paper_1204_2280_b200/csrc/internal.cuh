@@ -1,0 +1,135 @@
+// Internal declarations shared by the stage translation units of libbonsai (CUDA, sm_100a only).
+// Nothing here is part of the C-ABI; see include/bonsai.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "bonsai.h"
+
+namespace bonsai {
+
+constexpr int kMaxLevel = BONSAI_MAX_LEVEL;
+constexpr uint32_t kNone = 0xFFFFFFFFu;
+constexpr uint32_t kLeafBit = 0x80000000u;
+
+// ---- radix sort geometry (sort.cu) -------------------------------------------------------------
+constexpr int kRadixBits = 10;             // one 30-bit key word = 3 digits -> 9 LSD passes for 90 bits
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kSortPasses = 9;
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 16;             // keys per thread per tile
+constexpr int kSortTile = kSortThreads * kSortItems;
+
+// ---- tree build geometry (tree.cu) -------------------------------------------------------------
+constexpr int kTreeThreads = 256;
+constexpr int kTreeItems = 4;
+constexpr int kTreeTile = kTreeThreads * kTreeItems;  // particles per block
+constexpr int kLevelSlots = 32;                       // levels 0..30, padded
+constexpr int kMaxNleaf = 64;
+
+// ---- walk geometry (walk.cu) -------------------------------------------------------------------
+constexpr int kWalkWarps = 8;              // warps per block, one group per warp at a time
+constexpr int kWalkStack = 512;            // traversal stack entries per warp (see walk.cu for the bound)
+constexpr int kMaxNcrit = 64;
+
+// Device-resident control block at the start of the workspace (zeroed by bonsai_create).
+struct Control {
+    float lo[3];               // root cube corner (R3)
+    float side_f;              // root cube side as fp32 (power of two, exact)
+    float scale;               // 2^30 / side (exact)
+    int status;                // sticky device status (0 or BONSAI_ECAPACITY)
+    double side;               // root cube side
+    uint32_t n_cells;
+    uint32_t n_groups;
+    uint32_t n_active;
+    uint32_t bbox_ticket;
+    uint32_t walk_ticket;      // dynamic group scheduler of the walk
+    uint32_t level_ticket;     // last-block-done counter of k_tree_scan_levels
+    uint32_t pad0[2];
+    uint32_t level_offsets[32];  // first cell of level L; [31] = n_cells
+    unsigned long long sum_pp;   // interaction totals of the last walk (sink-source pairs)
+    unsigned long long sum_pc;
+};
+
+// Walk layout of a cell, two 32-byte records (one DRAM/L2 sector each):
+//   CellMac : what the opening test and the monopole need + the links
+//   CellQuad: what only an accepted cell needs
+struct __align__(16) CellMac {
+    float cx, cy, cz, m;       // centre of mass, mass (fp32, rounded once from fp64)
+    float delta, lside;        // |COM - geometric centre|, geometric side
+    uint32_t first;            // internal: first child;  leaf: first sorted particle
+    uint32_t info;             // internal: n_child (1..8);  leaf: kLeafBit | count
+};
+struct __align__(16) CellQuad {
+    float xx, yy, zz, xy, xz, yz;  // raw second moments about the COM
+    float mtr_half;                // -1/2 (xx + yy + zz)
+    float mtr_3half;               // -3/2 (xx + yy + zz)
+};
+
+struct Buffers {
+    Control* ctl;
+    // sort: ping-pong key records, structure of arrays
+    uint32_t* key[2][3];       // [buffer][word]: hi, mid, lo
+    uint32_t* idx[2];
+    uint32_t* ghist;           // [kSortPasses][kRadix] global digit histograms -> exclusive bases
+    uint32_t* tile_count;      // [kRadix][n_tiles] per-tile digit counts -> exclusive prefix over tiles
+    float* bbox_partial;       // [blocks][6]
+    float4* sorted_pos;
+    // tree
+    int8_t* lcp;               // [n+1] common leading digits of key[i-1], key[i]; -1 at both ends
+    int8_t* leaf_level;        // [n] level of the leaf containing particle i
+    uint32_t* blk_level_count; // [kLevelSlots][n_blocks] cells per level per block -> exclusive prefix over blocks
+    uint32_t* level_total;     // [kLevelSlots]
+    uint32_t *c_level, *c_first, *c_count, *c_first_child, *c_n_child, *c_parent;
+    // multipoles
+    CellMac* c_mac;            // [cap]
+    CellQuad* c_quad;          // [cap]
+    double* c_mom;             // [cap][10] fp64: M, COMx, COMy, COMz, Qxx, Qyy, Qzz, Qxy, Qxz, Qyz
+    uint32_t* c_arrived;       // [cap] children that have finished
+    // groups
+    uint32_t* rank;            // [n+1] exclusive count of active particles (sorted order)
+    uint32_t* active_list;     // [n]
+    uint32_t* g_flag;          // [n+1] scan scratch (mode 0: 1 where a non-empty group starts)
+    uint32_t* g_cell;          // [n] mode 0: 1 + id of the group cell starting at particle i (0 = none)
+    uint32_t *g_first, *g_count;
+    float *g_bmin, *g_bmax;
+    uint32_t* scan_tmp;        // block sums of the device-wide scan
+    // walk
+    uint32_t *n_pp, *n_pc;     // [n] load order
+};
+
+struct Ctx {
+    uint32_t n_max, n;
+    bonsai_params prm;
+    uint32_t cap_cells;
+    cudaStream_t stream;
+    Buffers b;
+    const float4* pos_mass;    // caller's particles (load order)
+    int sorted_buf;            // which ping-pong buffer holds the sorted keys
+    int state;                 // 0 created, 1 loaded, 2 tree built, 3 multipoles done, 4 walked
+    bool groups_all_active;    // the group list on the device is the all-active one
+    bool timing;
+    cudaEvent_t ev[BONSAI_N_STAGES][2];
+    bool ev_valid[BONSAI_N_STAGES];
+    uint64_t launches;
+    int num_sms;
+};
+
+inline uint32_t div_up(uint32_t a, uint32_t b) { return (a + b - 1) / b; }
+
+// Stage entry points (each enqueues kernels on ctx->stream and bumps ctx->launches).
+cudaError_t stage_bbox(Ctx* c);
+cudaError_t stage_keys(Ctx* c);
+cudaError_t stage_sort(Ctx* c);
+cudaError_t stage_reorder(Ctx* c);
+cudaError_t stage_build(Ctx* c);
+cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order);
+cudaError_t stage_multipoles(Ctx* c);
+cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out);
+size_t walk_smem_bytes(uint32_t nleaf);
+
+// Device-wide exclusive scan of u32 (scan.cu): out[i] = sum_{j<i} in[j], i in [0, n]; out has n+1 entries
+// (out[n] = total).  in may alias out.  tmp needs div_up(n, 2048) + 1 entries.
+cudaError_t exclusive_scan_u32(Ctx* c, const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* tmp);
+
+}  // namespace bonsai
