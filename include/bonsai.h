@@ -129,10 +129,12 @@ typedef struct {
     const uint32_t* first_child;   /*   0 for a leaf                                                    */
     const uint32_t* n_child;       /*   0 for a leaf                                                    */
     const uint32_t* parent;        /*   0xFFFFFFFF for the root                                         */
-    const float* com_m;            /* device float4[cap]: COM x, y, z, mass (after multipoles)          */
-    const float* quad;             /* device float[6*cap]: xx, yy, zz, xy, xz, yz                       */
-    const float* delta;            /* device float[cap]                                                 */
-    const float* lside;            /* device float[cap]                                                 */
+    const float* mac;              /* device, 8 x 4 bytes per cell (after multipoles; the walk's layout):
+                                      f32 COM x, y, z, mass, delta = |COM - geometric centre|, l = cell side,
+                                      then u32 link (leaf: first particle; else first child) and u32 info
+                                      (leaf: 0x80000000 | count; else n_child)                                */
+    const float* quad;             /* device, 8 floats per cell: xx, yy, zz, xy, xz, yz (raw second moments
+                                      about the COM, R8), then -tr/2 and -3 tr/2 as the walk uses them       */
 } bonsai_cells_view;
 int bonsai_get_cells(bonsai_ctx* ctx, bonsai_cells_view* out);
 
@@ -151,6 +153,9 @@ int bonsai_get_groups(bonsai_ctx* ctx, bonsai_groups_view* out);
 /* Interaction counts of the last walk, per particle in LOAD order (R21): n_pp = particles in the opened
  * leaves of the particle's group minus itself, n_pc = accepted cells of its group. */
 int bonsai_get_counts(bonsai_ctx* ctx, const uint32_t** n_pp_dev, const uint32_t** n_pc_dev);
+
+/* Totals of the last walk over all sinks: sum of n_pp and of n_pc (R21).  Waits for the stream. */
+int bonsai_get_interaction_totals(bonsai_ctx* ctx, uint64_t* sum_pp, uint64_t* sum_pc);
 
 /* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events between stages from then on;
  * bonsai_get_stage_ms() waits for the stream and writes milliseconds of the most recent execution of each

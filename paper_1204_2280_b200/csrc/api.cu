@@ -1,0 +1,361 @@
+// The C-ABI of libbonsai (include/bonsai.h): context, workspace carve-up, call sequencing, introspection.
+// No arithmetic of the method lives here; each call enqueues the stage kernels of sort.cu / tree.cu /
+// groups.cu / multipoles.cu / walk.cu on the caller's stream.
+#include <cmath>
+#include <new>
+
+#include "internal.cuh"
+
+using namespace bonsai;
+
+struct bonsai_ctx {
+    Ctx c;
+};
+
+namespace {
+
+constexpr size_t kAlign = 256;
+
+struct Carver {
+    unsigned char* base;
+    size_t off = 0;
+    template <typename T>
+    T* take(size_t count) {
+        off = (off + kAlign - 1) / kAlign * kAlign;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += sizeof(T) * count;
+        return p;
+    }
+};
+
+bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out) {
+    bonsai_params p;
+    p.nleaf = 16; p.ncrit = 64; p.group_mode = 1; p.cap_cells = 0;
+    if (in) {
+        if (in->nleaf) p.nleaf = in->nleaf;
+        if (in->ncrit) p.ncrit = in->ncrit;
+        p.group_mode = in->group_mode;
+        p.cap_cells = in->cap_cells;
+    }
+    if (p.cap_cells == 0) {
+        unsigned long long cap = 2ull * n_max + 256ull;
+        if (cap >= (1ull << 29)) cap = (1ull << 29) - 1;
+        p.cap_cells = (uint32_t)cap;
+    }
+    if (n_max == 0 || n_max > (1u << 30)) return false;
+    if (p.nleaf < 1 || p.nleaf > (uint32_t)kMaxNleaf) return false;
+    if (p.ncrit < 1 || p.ncrit > (uint32_t)kMaxNcrit) return false;
+    if (p.group_mode > 1) return false;
+    if (p.cap_cells < 1 || p.cap_cells >= (1u << 29)) return false;  // walk stack entries pack the id into 29 bits
+    *out = p;
+    return true;
+}
+
+// Lays the buffers out in the workspace; with base = nullptr it only measures.
+size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b) {
+    Carver cv{base};
+    const size_t cap = p.cap_cells;
+    const uint32_t n_tiles = div_up(n, kSortTile);
+    const uint32_t n_tblocks = div_up(n + 1, kTreeTile);
+    Buffers t{};
+    t.ctl = cv.take<Control>(1);
+    for (int k = 0; k < 2; ++k) {
+        for (int w = 0; w < 3; ++w) t.key[k][w] = cv.take<uint32_t>(n);
+        t.idx[k] = cv.take<uint32_t>(n);
+    }
+    t.ghist = cv.take<uint32_t>((size_t)kSortPasses * kRadix);
+    t.tile_count = cv.take<uint32_t>((size_t)kRadix * n_tiles);
+    t.bbox_partial = cv.take<float>(6 * 148 * 16);
+    t.sorted_pos = cv.take<float4>(n);
+    t.lcp = cv.take<int8_t>((size_t)n + 1);
+    t.leaf_level = cv.take<int8_t>((size_t)n + 1);
+    t.blk_level_count = cv.take<uint32_t>((size_t)kLevelSlots * n_tblocks);
+    t.level_total = cv.take<uint32_t>(kLevelSlots);
+    t.c_level = cv.take<uint32_t>(cap);
+    t.c_first = cv.take<uint32_t>(cap);
+    t.c_count = cv.take<uint32_t>(cap);
+    t.c_first_child = cv.take<uint32_t>(cap);
+    t.c_n_child = cv.take<uint32_t>(cap);
+    t.c_parent = cv.take<uint32_t>(cap);
+    t.c_mac = cv.take<CellMac>(cap);
+    t.c_quad = cv.take<CellQuad>(cap);
+    t.c_mom = cv.take<double>(cap * 10);
+    t.c_arrived = cv.take<uint32_t>(cap);
+    t.rank = cv.take<uint32_t>((size_t)n + 1);
+    t.active_list = cv.take<uint32_t>(n);
+    t.g_flag = cv.take<uint32_t>((size_t)n + 1);
+    t.g_cell = cv.take<uint32_t>(n);
+    const size_t max_groups = (p.group_mode == 1) ? div_up(n, p.ncrit) : n;
+    t.g_first = cv.take<uint32_t>(max_groups);
+    t.g_count = cv.take<uint32_t>(max_groups);
+    t.g_bmin = cv.take<float>(3 * max_groups);
+    t.g_bmax = cv.take<float>(3 * max_groups);
+    t.scan_tmp = cv.take<uint32_t>((size_t)div_up(n + 1, 2048) + 2);
+    t.n_pp = cv.take<uint32_t>(n);
+    t.n_pc = cv.take<uint32_t>(n);
+    if (b) *b = t;
+    return (cv.off + kAlign - 1) / kAlign * kAlign;
+}
+
+struct StageTimer {
+    Ctx* c;
+    int stage;
+    StageTimer(Ctx* c_, int s) : c(c_), stage(s) {
+        if (c->timing) cudaEventRecord(c->ev[stage][0], c->stream);
+    }
+    ~StageTimer() {
+        if (c->timing) {
+            cudaEventRecord(c->ev[stage][1], c->stream);
+            c->ev_valid[stage] = true;
+        }
+    }
+};
+
+#define BONSAI_TRY(expr)                                  \
+    do {                                                  \
+        cudaError_t e_ = (expr);                          \
+        if (e_ != cudaSuccess) return BONSAI_ECUDA;       \
+    } while (0)
+
+}  // namespace
+
+extern "C" {
+
+size_t bonsai_workspace_bytes(uint32_t n_max, const bonsai_params* params) {
+    bonsai_params p;
+    if (!resolve_params(n_max, params, &p)) return 0;
+    return carve(nullptr, n_max, p, nullptr);
+}
+
+int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_dev, size_t workspace_bytes,
+                  void* cuda_stream, bonsai_ctx** out) {
+    if (!out) return BONSAI_EINVAL;
+    *out = nullptr;
+    bonsai_params p;
+    if (!resolve_params(n_max, params, &p)) return BONSAI_EINVAL;
+    if (!workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) % kAlign) != 0) return BONSAI_EINVAL;
+    if (workspace_bytes < carve(nullptr, n_max, p, nullptr)) return BONSAI_ENOMEM;
+    bonsai_ctx* h = new (std::nothrow) bonsai_ctx();
+    if (!h) return BONSAI_ENOMEM;
+    Ctx& c = h->c;
+    c.n_max = n_max;
+    c.n = 0;
+    c.prm = p;
+    c.cap_cells = p.cap_cells;
+    c.stream = static_cast<cudaStream_t>(cuda_stream);
+    carve(static_cast<unsigned char*>(workspace_dev), n_max, p, &c.b);
+    c.pos_mass = nullptr;
+    c.sorted_buf = 0;
+    c.state = 0;
+    c.groups_all_active = false;
+    c.timing = false;
+    c.launches = 0;
+    for (int s = 0; s < BONSAI_N_STAGES; ++s) {
+        c.ev_valid[s] = false;
+        c.ev[s][0] = c.ev[s][1] = nullptr;
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&c.num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete h;
+        return BONSAI_ECUDA;
+    }
+    // control block and the self-cleaning arrival counters start at zero
+    if (cudaMemsetAsync(c.b.ctl, 0, sizeof(Control), c.stream) != cudaSuccess ||
+        cudaMemsetAsync(c.b.c_arrived, 0, sizeof(uint32_t) * (size_t)c.cap_cells, c.stream) != cudaSuccess) {
+        delete h;
+        return BONSAI_ECUDA;
+    }
+    *out = h;
+    return BONSAI_OK;
+}
+
+int bonsai_load(bonsai_ctx* h, const float* pos_mass_dev, uint32_t n) {
+    if (!h || !pos_mass_dev) return BONSAI_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(pos_mass_dev) % 16) != 0) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max) return BONSAI_EINVAL;
+    h->c.pos_mass = reinterpret_cast<const float4*>(pos_mass_dev);
+    h->c.n = n;
+    h->c.state = 1;
+    return BONSAI_OK;
+}
+
+int bonsai_build_tree(bonsai_ctx* h) {
+    if (!h) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    if (c->state < 1) return BONSAI_ESTATE;
+    { StageTimer t(c, 0); BONSAI_TRY(stage_bbox(c)); }
+    { StageTimer t(c, 1); BONSAI_TRY(stage_keys(c)); }
+    { StageTimer t(c, 2); BONSAI_TRY(stage_sort(c)); }
+    { StageTimer t(c, 3); BONSAI_TRY(stage_reorder(c)); }
+    { StageTimer t(c, 4); BONSAI_TRY(stage_build(c)); }
+    { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
+    c->state = 2;
+    return BONSAI_OK;
+}
+
+int bonsai_compute_multipoles(bonsai_ctx* h) {
+    if (!h) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    if (c->state < 2) return BONSAI_ESTATE;
+    { StageTimer t(c, 6); BONSAI_TRY(stage_multipoles(c)); }
+    c->state = 3;
+    return BONSAI_OK;
+}
+
+int bonsai_walk(bonsai_ctx* h, float theta, float eps, const uint8_t* active_mask_dev, float* acc_pot_dev_out) {
+    if (!h || !acc_pot_dev_out) return BONSAI_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(acc_pot_dev_out) % 16) != 0) return BONSAI_EINVAL;
+    if (!(theta >= 0.0f) || !(eps >= 0.0f) || std::isinf(theta) || std::isinf(eps)) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    if (c->state < 3) return BONSAI_ESTATE;
+    if (active_mask_dev != nullptr || !c->groups_all_active) {
+        StageTimer t(c, 5);
+        BONSAI_TRY(stage_groups(c, active_mask_dev));
+    }
+    { StageTimer t(c, 7); BONSAI_TRY(stage_walk(c, theta, eps, reinterpret_cast<float4*>(acc_pot_dev_out))); }
+    c->state = 4;
+    return BONSAI_OK;
+}
+
+void bonsai_destroy(bonsai_ctx* h) {
+    if (!h) return;
+    for (int s = 0; s < BONSAI_N_STAGES; ++s)
+        for (int k = 0; k < 2; ++k)
+            if (h->c.ev[s][k]) cudaEventDestroy(h->c.ev[s][k]);
+    delete h;
+}
+
+int bonsai_sync(bonsai_ctx* h) {
+    if (!h) return BONSAI_EINVAL;
+    int status = 0;
+    if (cudaMemcpyAsync(&status, &h->c.b.ctl->status, sizeof(int), cudaMemcpyDeviceToHost, h->c.stream) != cudaSuccess)
+        return BONSAI_ECUDA;
+    if (cudaStreamSynchronize(h->c.stream) != cudaSuccess) return BONSAI_ECUDA;
+    return status;
+}
+
+// ---- introspection ---------------------------------------------------------------------------------
+
+int bonsai_get_box(bonsai_ctx* h, const float** box4_dev) {
+    if (!h || !box4_dev) return BONSAI_EINVAL;
+    if (h->c.state < 2) return BONSAI_ESTATE;
+    *box4_dev = h->c.b.ctl->lo;  // lo[3] followed by side_f
+    return BONSAI_OK;
+}
+
+int bonsai_get_keys(bonsai_ctx* h, const uint32_t** hi_dev, const uint32_t** mid_dev, const uint32_t** lo_dev) {
+    if (!h || !hi_dev || !mid_dev || !lo_dev) return BONSAI_EINVAL;
+    if (h->c.state < 2) return BONSAI_ESTATE;
+    const int s = h->c.sorted_buf;
+    *hi_dev = h->c.b.key[s][0];
+    *mid_dev = h->c.b.key[s][1];
+    *lo_dev = h->c.b.key[s][2];
+    return BONSAI_OK;
+}
+
+int bonsai_get_perm(bonsai_ctx* h, const uint32_t** perm_dev) {
+    if (!h || !perm_dev) return BONSAI_EINVAL;
+    if (h->c.state < 2) return BONSAI_ESTATE;
+    *perm_dev = h->c.b.idx[h->c.sorted_buf];
+    return BONSAI_OK;
+}
+
+int bonsai_get_sorted_pos(bonsai_ctx* h, const float** pos_mass_dev) {
+    if (!h || !pos_mass_dev) return BONSAI_EINVAL;
+    if (h->c.state < 2) return BONSAI_ESTATE;
+    *pos_mass_dev = reinterpret_cast<const float*>(h->c.b.sorted_pos);
+    return BONSAI_OK;
+}
+
+int bonsai_get_cells(bonsai_ctx* h, bonsai_cells_view* out) {
+    if (!h || !out) return BONSAI_EINVAL;
+    if (h->c.state < 2) return BONSAI_ESTATE;
+    const Buffers& b = h->c.b;
+    out->cap_cells = h->c.cap_cells;
+    out->n_cells = &b.ctl->n_cells;
+    out->level_offsets = b.ctl->level_offsets;
+    out->level = b.c_level;
+    out->first = b.c_first;
+    out->count = b.c_count;
+    out->first_child = b.c_first_child;
+    out->n_child = b.c_n_child;
+    out->parent = b.c_parent;
+    out->mac = reinterpret_cast<const float*>(b.c_mac);
+    out->quad = reinterpret_cast<const float*>(b.c_quad);
+    return BONSAI_OK;
+}
+
+int bonsai_get_groups(bonsai_ctx* h, bonsai_groups_view* out) {
+    if (!h || !out) return BONSAI_EINVAL;
+    if (h->c.state < 2) return BONSAI_ESTATE;
+    const Buffers& b = h->c.b;
+    out->n_groups = &b.ctl->n_groups;
+    out->n_active = &b.ctl->n_active;
+    out->active_list = b.active_list;
+    out->first = b.g_first;
+    out->count = b.g_count;
+    out->bmin = b.g_bmin;
+    out->bmax = b.g_bmax;
+    return BONSAI_OK;
+}
+
+int bonsai_get_counts(bonsai_ctx* h, const uint32_t** n_pp_dev, const uint32_t** n_pc_dev) {
+    if (!h || !n_pp_dev || !n_pc_dev) return BONSAI_EINVAL;
+    if (h->c.state < 4) return BONSAI_ESTATE;
+    *n_pp_dev = h->c.b.n_pp;
+    *n_pc_dev = h->c.b.n_pc;
+    return BONSAI_OK;
+}
+
+int bonsai_get_interaction_totals(bonsai_ctx* h, uint64_t* sum_pp, uint64_t* sum_pc) {
+    if (!h || !sum_pp || !sum_pc) return BONSAI_EINVAL;
+    if (h->c.state < 4) return BONSAI_ESTATE;
+    unsigned long long v[2] = {0, 0};
+    if (cudaMemcpyAsync(v, &h->c.b.ctl->sum_pp, sizeof(v), cudaMemcpyDeviceToHost, h->c.stream) != cudaSuccess)
+        return BONSAI_ECUDA;
+    if (cudaStreamSynchronize(h->c.stream) != cudaSuccess) return BONSAI_ECUDA;
+    *sum_pp = v[0];
+    *sum_pc = v[1];
+    return BONSAI_OK;
+}
+
+int bonsai_set_timing(bonsai_ctx* h, int enable) {
+    if (!h) return BONSAI_EINVAL;
+    Ctx& c = h->c;
+    if (enable && !c.ev[0][0]) {
+        for (int s = 0; s < BONSAI_N_STAGES; ++s)
+            for (int k = 0; k < 2; ++k)
+                if (cudaEventCreate(&c.ev[s][k]) != cudaSuccess) return BONSAI_ECUDA;
+    }
+    c.timing = enable != 0;
+    return BONSAI_OK;
+}
+
+int bonsai_get_stage_ms(bonsai_ctx* h, float out_ms[BONSAI_N_STAGES]) {
+    if (!h || !out_ms) return BONSAI_EINVAL;
+    Ctx& c = h->c;
+    if (cudaStreamSynchronize(c.stream) != cudaSuccess) return BONSAI_ECUDA;
+    for (int s = 0; s < BONSAI_N_STAGES; ++s) {
+        out_ms[s] = 0.0f;
+        if (c.ev_valid[s] && cudaEventElapsedTime(&out_ms[s], c.ev[s][0], c.ev[s][1]) != cudaSuccess)
+            return BONSAI_ECUDA;
+    }
+    return BONSAI_OK;
+}
+
+uint64_t bonsai_get_launch_count(bonsai_ctx* h) { return h ? h->c.launches : 0; }
+
+const char* bonsai_strerror(int code) {
+    switch (code) {
+        case BONSAI_OK: return "ok";
+        case BONSAI_EINVAL: return "invalid argument";
+        case BONSAI_ESTATE: return "call out of order";
+        case BONSAI_ECAPACITY: return "cell capacity or traversal stack exceeded";
+        case BONSAI_ECUDA: return "CUDA runtime error";
+        case BONSAI_ENOMEM: return "workspace too small";
+        default: return "unknown error";
+    }
+}
+
+}  // extern "C"

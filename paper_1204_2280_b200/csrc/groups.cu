@@ -1,0 +1,158 @@
+// Stage a4': walk groups (the traversal follows "the method used for tree-traversion on vector
+// machines (Barnes 1990)" -- one shared traversal per group of neighbouring particles; readings R13, R19).
+//
+//   rank[i]        exclusive count of ACTIVE particles among sorted particles 0..i-1  (rank[n] = n_active)
+//   active_list[k] sorted index of the k-th active particle
+//   mode 1 (sorted chunks): group g = active particles [g ncrit, min((g+1) ncrit, n_active))
+//   mode 0 (tree cells):    the cells with count <= ncrit (or childless) whose parent has count > ncrit, in key
+//                           order, each keeping only its active members, dropped when none remain
+//   bmin / bmax            exact fp32 per-axis min / max over the group's members
+#include "internal.cuh"
+
+namespace bonsai {
+
+__global__ void __launch_bounds__(256) k_groups_identity(uint32_t n, uint32_t* __restrict__ rank,
+                                                         uint32_t* __restrict__ active_list, Control* __restrict__ ctl) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) active_list[i] = i;
+    if (i <= n) rank[i] = i;
+    if (i == 0) ctl->n_active = n;
+}
+
+// flags in sorted order from a mask in load order
+__global__ void __launch_bounds__(256) k_groups_flags(const uint8_t* __restrict__ mask, const uint32_t* __restrict__ perm,
+                                                      uint32_t n, uint32_t* __restrict__ flag) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) flag[i] = mask[__ldg(&perm[i])] ? 1u : 0u;
+}
+
+__global__ void __launch_bounds__(256) k_groups_compact(const uint32_t* __restrict__ rank, uint32_t n,
+                                                        uint32_t* __restrict__ active_list, Control* __restrict__ ctl) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        const uint32_t r = rank[i];
+        if (rank[i + 1] != r) active_list[r] = i;
+    }
+    if (i == 0) ctl->n_active = rank[n];
+}
+
+// mode 1: first / count of every chunk
+__global__ void __launch_bounds__(256) k_groups_chunks(const uint32_t* __restrict__ rank, uint32_t n, uint32_t ncrit,
+                                                       uint32_t* __restrict__ g_first, uint32_t* __restrict__ g_count,
+                                                       Control* __restrict__ ctl) {
+    const uint32_t na = rank[n];
+    const uint32_t ng = (na + ncrit - 1) / ncrit;
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g == 0) ctl->n_groups = ng;
+    if (g >= ng) return;
+    g_first[g] = g * ncrit;
+    g_count[g] = min(ncrit, na - g * ncrit);
+}
+
+// mode 0, step 1: mark the first particle of every non-empty group cell
+__global__ void __launch_bounds__(256) k_groups_mark(const Control* __restrict__ ctl, uint32_t cap_cells, uint32_t ncrit,
+                                                     const uint32_t* __restrict__ c_first,
+                                                     const uint32_t* __restrict__ c_count,
+                                                     const uint32_t* __restrict__ c_n_child,
+                                                     const uint32_t* __restrict__ c_parent,
+                                                     const uint32_t* __restrict__ rank, uint32_t* __restrict__ g_flag,
+                                                     uint32_t* __restrict__ g_cell) {
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= min(ctl->n_cells, cap_cells)) return;
+    const uint32_t cnt = c_count[c];
+    if (!(cnt <= ncrit || c_n_child[c] == 0)) return;
+    const uint32_t p = c_parent[c];
+    if (p != kNone && c_count[p] <= ncrit) return;  // an ancestor already is the group
+    const uint32_t f = c_first[c];
+    if (rank[f + cnt] == rank[f]) return;            // no active member
+    g_flag[f] = 1u;
+    g_cell[f] = c + 1u;
+}
+
+// mode 0, step 2 (after the scan of g_flag): first / count of every group
+__global__ void __launch_bounds__(256) k_groups_cells(const uint32_t* __restrict__ g_index,
+                                                      const uint32_t* __restrict__ g_cell, uint32_t n,
+                                                      const uint32_t* __restrict__ c_count,
+                                                      const uint32_t* __restrict__ rank, uint32_t* __restrict__ g_first,
+                                                      uint32_t* __restrict__ g_count, Control* __restrict__ ctl) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) ctl->n_groups = g_index[n];
+    if (i >= n) return;
+    const uint32_t c1 = g_cell[i];
+    if (c1 == 0) return;
+    const uint32_t g = g_index[i];
+    const uint32_t r0 = rank[i];
+    g_first[g] = r0;
+    g_count[g] = rank[i + c_count[c1 - 1]] - r0;
+}
+
+// one warp per group (grid-stride): exact fp32 box
+__global__ void __launch_bounds__(256) k_groups_box(const Control* __restrict__ ctl, const uint32_t* __restrict__ g_first,
+                                                    const uint32_t* __restrict__ g_count,
+                                                    const uint32_t* __restrict__ active_list,
+                                                    const float4* __restrict__ sorted_pos, float* __restrict__ g_bmin,
+                                                    float* __restrict__ g_bmax) {
+    const uint32_t ng = ctl->n_groups;
+    const int l = threadIdx.x & 31;
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; g < ng; g += warps) {
+        const uint32_t f = g_first[g], cnt = g_count[g];
+        float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+        for (uint32_t k = l; k < cnt; k += 32) {
+            const float4 p = __ldg(&sorted_pos[__ldg(&active_list[f + k])]);
+            mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
+            mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
+            mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                mn[a] = fminf(mn[a], __shfl_xor_sync(0xFFFFFFFFu, mn[a], o));
+                mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xFFFFFFFFu, mx[a], o));
+            }
+        if (l < 3) {
+            g_bmin[3 * g + l] = (l == 0) ? mn[0] : (l == 1) ? mn[1] : mn[2];
+            g_bmax[3 * g + l] = (l == 0) ? mx[0] : (l == 1) ? mx[1] : mx[2];
+        }
+    }
+}
+
+cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order) {
+    const uint32_t n = c->n;
+    Buffers& b = c->b;
+    cudaError_t e;
+    if (mask_load_order == nullptr) {
+        k_groups_identity<<<div_up(n + 1, 256), 256, 0, c->stream>>>(n, b.rank, b.active_list, b.ctl);
+        c->launches += 1;
+    } else {
+        k_groups_flags<<<div_up(n, 256), 256, 0, c->stream>>>(mask_load_order, b.idx[c->sorted_buf], n, b.rank);
+        c->launches += 1;
+        if ((e = exclusive_scan_u32(c, b.rank, b.rank, n, b.scan_tmp)) != cudaSuccess) return e;
+        k_groups_compact<<<div_up(n, 256), 256, 0, c->stream>>>(b.rank, n, b.active_list, b.ctl);
+        c->launches += 1;
+    }
+    if (c->prm.group_mode == 1) {
+        k_groups_chunks<<<div_up(div_up(n, c->prm.ncrit), 256), 256, 0, c->stream>>>(b.rank, n, c->prm.ncrit, b.g_first,
+                                                                                   b.g_count, b.ctl);
+        c->launches += 1;
+    } else {
+        if ((e = cudaMemsetAsync(b.g_flag, 0, sizeof(uint32_t) * (size_t)(n + 1), c->stream)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(b.g_cell, 0, sizeof(uint32_t) * (size_t)n, c->stream)) != cudaSuccess) return e;
+        k_groups_mark<<<div_up(c->cap_cells, 256), 256, 0, c->stream>>>(b.ctl, c->cap_cells, c->prm.ncrit, b.c_first,
+                                                                        b.c_count, b.c_n_child, b.c_parent, b.rank,
+                                                                        b.g_flag, b.g_cell);
+        c->launches += 1;
+        if ((e = exclusive_scan_u32(c, b.g_flag, b.g_flag, n, b.scan_tmp)) != cudaSuccess) return e;
+        k_groups_cells<<<div_up(n, 256), 256, 0, c->stream>>>(b.g_flag, b.g_cell, n, b.c_count, b.rank, b.g_first,
+                                                              b.g_count, b.ctl);
+        c->launches += 1;
+    }
+    k_groups_box<<<c->num_sms * 8, 256, 0, c->stream>>>(b.ctl, b.g_first, b.g_count, b.active_list, b.sorted_pos,
+                                                        b.g_bmin, b.g_bmax);
+    c->launches += 1;
+    c->groups_all_active = (mask_load_order == nullptr);
+    return cudaGetLastError();
+}
+
+}  // namespace bonsai

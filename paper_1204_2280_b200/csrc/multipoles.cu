@@ -1,0 +1,171 @@
+// Stage a5: multipole moments ("computation of the tree-properties (multipole moments)", P:L30;
+// BASELINE.json north_star: monopole + quadrupole; reading R8 of DESIGN.md).
+//
+// Per cell: M, centre of mass, the 6 raw second moments about the centre of mass, delta = |COM - geometric
+// centre| and the geometric side l.  Everything is accumulated in fp64 and rounded ONCE to fp32, because the
+// fp32 opening test of the walk must see the same COM / delta as the reference to the last bit (R9).
+//
+// One launch, bottom-up without level barriers: a thread per cell; leaves sum their particles (in particle order,
+// without FMA contraction), then every thread climbs: it bumps its parent's arrival counter and the LAST child
+// to arrive combines the children's fp64 moments (parallel-axis shift about the parent's COM; moments about
+// the origin would cancel catastrophically in the halo) and continues upward.  Nobody waits on anybody.
+#include "internal.cuh"
+
+namespace bonsai {
+
+__device__ __forceinline__ uint32_t compact10(uint32_t v) {  // every third bit of 30 -> 10 bits
+    v &= 0x09249249u;
+    v = (v | (v >> 2)) & 0x030C30C3u;
+    v = (v | (v >> 4)) & 0x0300F00Fu;
+    v = (v | (v >> 8)) & 0x030000FFu;
+    v = (v | (v >> 16)) & 0x3FFu;
+    return v;
+}
+
+struct Mom {
+    double m, cx, cy, cz, xx, yy, zz, xy, xz, yz;
+};
+
+__device__ __forceinline__ void store_cell(const Mom& q, uint32_t c, int L, uint32_t khi, uint32_t kmid, uint32_t klo,
+                                           const Control* __restrict__ ctl, uint32_t link_first, uint32_t link_info,
+                                           double* __restrict__ c_mom, CellMac* __restrict__ c_mac,
+                                           CellQuad* __restrict__ c_quad) {
+    // geometric centre: integer cell coordinate = top L bits of the quantised coordinate of any member (R8)
+    const double l = ldexp(ctl->side, -L);
+    double g[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int sh = 2 - a;
+        const uint32_t qa = (compact10(khi >> sh) << 20) | (compact10(kmid >> sh) << 10) | compact10(klo >> sh);
+        const uint32_t ca = (L == 0) ? 0u : (qa >> (kMaxLevel - L));
+        g[a] = __dadd_rn((double)ctl->lo[a], __dmul_rn(__dadd_rn((double)ca, 0.5), l));
+    }
+    Mom o = q;
+    if (!(q.m > 0.0)) {  // only zero-mass members: COM is undefined, take the geometric centre (R8)
+        o.cx = g[0]; o.cy = g[1]; o.cz = g[2];
+        o.xx = o.yy = o.zz = o.xy = o.xz = o.yz = 0.0;
+    }
+    const double ex = __dadd_rn(o.cx, -g[0]), ey = __dadd_rn(o.cy, -g[1]), ez = __dadd_rn(o.cz, -g[2]);
+    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+    double* mo = c_mom + (size_t)c * 10;
+    __stcg(&mo[0], o.m); __stcg(&mo[1], o.cx); __stcg(&mo[2], o.cy); __stcg(&mo[3], o.cz);
+    __stcg(&mo[4], o.xx); __stcg(&mo[5], o.yy); __stcg(&mo[6], o.zz);
+    __stcg(&mo[7], o.xy); __stcg(&mo[8], o.xz); __stcg(&mo[9], o.yz);
+    CellMac cm;
+    cm.cx = (float)o.cx; cm.cy = (float)o.cy; cm.cz = (float)o.cz; cm.m = (float)o.m;
+    cm.delta = (float)sqrt(d2);
+    cm.lside = (float)l;
+    cm.first = link_first;
+    cm.info = link_info;
+    c_mac[c] = cm;
+    CellQuad cq;
+    cq.xx = (float)o.xx; cq.yy = (float)o.yy; cq.zz = (float)o.zz;
+    cq.xy = (float)o.xy; cq.xz = (float)o.xz; cq.yz = (float)o.yz;
+    const float tr = (cq.xx + cq.yy) + cq.zz;
+    cq.mtr_half = -0.5f * tr;
+    cq.mtr_3half = -1.5f * tr;
+    c_quad[c] = cq;
+}
+
+struct TreeView {
+    const uint32_t *level, *first, *count, *first_child, *n_child, *parent;
+};
+
+__global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ ctl, uint32_t cap_cells, TreeView t,
+                                                    const float4* __restrict__ sorted_pos,
+                                                    const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
+                                                    const uint32_t* __restrict__ klo, double* __restrict__ c_mom,
+                                                    CellMac* __restrict__ c_mac, CellQuad* __restrict__ c_quad,
+                                                    uint32_t* __restrict__ c_arrived) {
+    uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= min(ctl->n_cells, cap_cells)) return;
+    if (t.n_child[c] != 0) return;  // internal cells are produced by their last child
+    {
+        const uint32_t f = t.first[c], cnt = t.count[c];
+        Mom q;
+        double sx = 0.0, sy = 0.0, sz = 0.0;
+        q.m = 0.0;
+        for (uint32_t k = 0; k < cnt; ++k) {
+            const float4 p = __ldg(&sorted_pos[f + k]);
+            const double m = (double)p.w;
+            q.m = __dadd_rn(q.m, m);
+            sx = __dadd_rn(sx, __dmul_rn(m, (double)p.x));
+            sy = __dadd_rn(sy, __dmul_rn(m, (double)p.y));
+            sz = __dadd_rn(sz, __dmul_rn(m, (double)p.z));
+        }
+        q.cx = q.cy = q.cz = 0.0;
+        q.xx = q.yy = q.zz = q.xy = q.xz = q.yz = 0.0;
+        if (q.m > 0.0) {
+            q.cx = sx / q.m; q.cy = sy / q.m; q.cz = sz / q.m;
+            for (uint32_t k = 0; k < cnt; ++k) {
+                const float4 p = __ldg(&sorted_pos[f + k]);
+                const double m = (double)p.w;
+                const double dx = __dadd_rn((double)p.x, -q.cx), dy = __dadd_rn((double)p.y, -q.cy),
+                             dz = __dadd_rn((double)p.z, -q.cz);
+                q.xx = __dadd_rn(q.xx, __dmul_rn(__dmul_rn(m, dx), dx));
+                q.yy = __dadd_rn(q.yy, __dmul_rn(__dmul_rn(m, dy), dy));
+                q.zz = __dadd_rn(q.zz, __dmul_rn(__dmul_rn(m, dz), dz));
+                q.xy = __dadd_rn(q.xy, __dmul_rn(__dmul_rn(m, dx), dy));
+                q.xz = __dadd_rn(q.xz, __dmul_rn(__dmul_rn(m, dx), dz));
+                q.yz = __dadd_rn(q.yz, __dmul_rn(__dmul_rn(m, dy), dz));
+            }
+        }
+        store_cell(q, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f, kLeafBit | cnt, c_mom,
+                   c_mac, c_quad);
+    }
+    for (;;) {
+        const uint32_t p = t.parent[c];
+        if (p == kNone) return;
+        __threadfence();  // this cell's moments are visible before the arrival is
+        const uint32_t nc = t.n_child[p];
+        if (atomicAdd(&c_arrived[p], 1u) + 1u != nc) return;
+        c_arrived[p] = 0;  // ready for the next step
+        __threadfence();
+        const uint32_t fc = t.first_child[p];
+        Mom q;
+        double sx = 0.0, sy = 0.0, sz = 0.0;
+        q.m = 0.0;
+        for (uint32_t k = 0; k < nc; ++k) {
+            const double* mo = c_mom + (size_t)(fc + k) * 10;
+            const double m = __ldcg(&mo[0]);
+            q.m += m;
+            sx += m * __ldcg(&mo[1]);
+            sy += m * __ldcg(&mo[2]);
+            sz += m * __ldcg(&mo[3]);
+        }
+        q.cx = q.cy = q.cz = 0.0;
+        q.xx = q.yy = q.zz = q.xy = q.xz = q.yz = 0.0;
+        if (q.m > 0.0) {
+            q.cx = sx / q.m; q.cy = sy / q.m; q.cz = sz / q.m;
+            for (uint32_t k = 0; k < nc; ++k) {
+                const double* mo = c_mom + (size_t)(fc + k) * 10;
+                const double m = __ldcg(&mo[0]);
+                if (!(m > 0.0)) continue;  // a massless child carries the geometric centre, not a COM
+                const double dx = __ldcg(&mo[1]) - q.cx, dy = __ldcg(&mo[2]) - q.cy, dz = __ldcg(&mo[3]) - q.cz;
+                q.xx += __ldcg(&mo[4]) + m * dx * dx;
+                q.yy += __ldcg(&mo[5]) + m * dy * dy;
+                q.zz += __ldcg(&mo[6]) + m * dz * dz;
+                q.xy += __ldcg(&mo[7]) + m * dx * dy;
+                q.xz += __ldcg(&mo[8]) + m * dx * dz;
+                q.yz += __ldcg(&mo[9]) + m * dy * dz;
+            }
+        }
+        const uint32_t f = t.first[p];
+        store_cell(q, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc, c_mom, c_mac,
+                   c_quad);
+        c = p;
+    }
+}
+
+cudaError_t stage_multipoles(Ctx* c) {
+    Buffers& b = c->b;
+    const int s = c->sorted_buf;
+    TreeView t{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
+    k_multipoles<<<div_up(c->cap_cells, 128), 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0],
+                                                                   b.key[s][1], b.key[s][2], b.c_mom, b.c_mac, b.c_quad,
+                                                                   b.c_arrived);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+}  // namespace bonsai

@@ -1,0 +1,361 @@
+// Stage a6 / a7: the tree-walk ("tree-traverse"; more than 90 % of the step at theta = 0.75).
+// Readings R9 (opening criterion, defined in fp32), R10 (softening), R11 (self term), R12 (potential),
+// R14 (accepted leaf = p-c), R19 (active mask), R21 (interaction counts) of DESIGN.md.
+//
+// One warp per group (Barnes 1990: one shared traversal per group of neighbouring particles), groups handed out
+// by an atomic ticket so consecutive (= spatially adjacent) groups run at the same time and share the cell
+// data they pull through L2 / L1.  Each lane holds one sink, or two when the group has more than 32.
+//
+// Traversal: a per-warp stack in shared memory whose entries are RUNS of sibling cells (first_child, n_child) --
+// children are consecutive in the breadth-first numbering, so one entry expands into up to 8 lanes.  Per round
+// the warp pops as many entries as fit into 32 cells, every lane applies the opening test to one cell, then
+//   accepted cell      -> ring buffer of cell ids      (flushed 32 at a time through the p-c kernel)
+//   rejected leaf      -> its particles -> ring buffer  (flushed 32 at a time through the p-p kernel)
+//   rejected internal  -> its child run is pushed.
+// Interaction kernels run in fp32 (FFMA + MUFU.RSQ); each batch of <= 32 sources is summed in fp32 starting
+// from zero and the batch total is added to an fp64 running total, which keeps the round-off of the long sum
+// out of the result at the cost of 4 DADD per 32 interactions.
+#include "internal.cuh"
+
+namespace bonsai {
+
+struct WalkArgs {
+    Control* ctl;
+    const CellMac* mac;
+    const CellQuad* quad;
+    const float4* pos;       // sorted particles
+    const uint32_t* perm;    // sorted -> load index
+    const uint32_t* active_list;
+    const uint32_t *g_first, *g_count;
+    const float *g_bmin, *g_bmax;
+    float inv_theta, eps2;
+    float4* out;             // load order
+    uint32_t *n_pp, *n_pc;   // load order
+};
+
+struct __align__(16) WarpSmem {
+    float4 pp[64];                 // ring of p-p sources
+    float4 pc[32][3];              // staged p-c sources: (cx,cy,cz,m) (xx,yy,zz,xy) (xz,yz,-tr/2,-3tr/2)
+    uint32_t stack[kWalkStack];    // runs of sibling cells: (first << 3) | (n - 1)
+    uint32_t pc_ids[64];           // ring of accepted cell ids
+    uint32_t leaf_first[32];
+    uint32_t leaf_pref[36];
+};
+
+size_t walk_smem_bytes(uint32_t) { return sizeof(WarpSmem) * kWalkWarps; }
+
+__device__ __forceinline__ float rsqrt_fast(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+template <int NS>
+struct Sinks {
+    float x[NS], y[NS], z[NS];
+    double ax[NS], ay[NS], az[NS], ph[NS];  // ph accumulates +sum m/r (negated on output)
+};
+
+template <int NS, bool kZeroEps>
+__device__ __forceinline__ void eval_pp(WarpSmem& S, uint32_t r0, int nb, float eps2, Sinks<NS>& s) {
+    float ax[NS], ay[NS], az[NS], ph[NS];
+#pragma unroll
+    for (int k = 0; k < NS; ++k) ax[k] = ay[k] = az[k] = ph[k] = 0.0f;
+#pragma unroll 4
+    for (int j = 0; j < nb; ++j) {
+        const float4 q = S.pp[(r0 + j) & 63];
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+            const float dx = q.x - s.x[k], dy = q.y - s.y[k], dz = q.z - s.z[k];
+            float rinv;
+            if (kZeroEps) {  // eps = 0: the self term (and only it, R11) has r = 0 and must drop out
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                rinv = (r2 > 0.0f) ? rsqrt_fast(r2) : 0.0f;
+            } else {         // eps > 0: the self term adds exactly m/eps to ph and 0 to a; removed at the end
+                rinv = rsqrt_fast(fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2))));
+            }
+            const float mr = q.w * rinv;
+            const float rinv2 = rinv * rinv;
+            const float mr3 = mr * rinv2;
+            ph[k] += mr;
+            ax[k] = fmaf(mr3, dx, ax[k]);
+            ay[k] = fmaf(mr3, dy, ay[k]);
+            az[k] = fmaf(mr3, dz, az[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+        s.ax[k] += (double)ax[k]; s.ay[k] += (double)ay[k]; s.az[k] += (double)az[k]; s.ph[k] += (double)ph[k];
+    }
+    __syncwarp();
+}
+
+template <int NS>
+__device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t r0, int nb, int lane, Sinks<NS>& s) {
+    if (lane < nb) {
+        const uint32_t c = S.pc_ids[(r0 + lane) & 63];
+        const float4* m = reinterpret_cast<const float4*>(a.mac + c);
+        const float4* q = reinterpret_cast<const float4*>(a.quad + c);
+        S.pc[lane][0] = __ldg(m);
+        S.pc[lane][1] = __ldg(q);
+        S.pc[lane][2] = __ldg(q + 1);
+    }
+    __syncwarp();
+    float ax[NS], ay[NS], az[NS], ph[NS];
+#pragma unroll
+    for (int k = 0; k < NS; ++k) ax[k] = ay[k] = az[k] = ph[k] = 0.0f;
+#pragma unroll 2
+    for (int j = 0; j < nb; ++j) {
+        const float4 c0 = S.pc[j][0], c1 = S.pc[j][1], c2 = S.pc[j][2];
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+            const float dx = c0.x - s.x[k], dy = c0.y - s.y[k], dz = c0.z - s.z[k];
+            const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.eps2)));
+            const float rinv = rsqrt_fast(r2);
+            const float rinv2 = rinv * rinv;
+            const float qrx = fmaf(c1.x, dx, fmaf(c1.w, dy, c2.x * dz));
+            const float qry = fmaf(c1.w, dx, fmaf(c1.y, dy, c2.y * dz));
+            const float qrz = fmaf(c2.x, dx, fmaf(c2.y, dy, c1.z * dz));
+            const float qq = fmaf(dx, qrx, fmaf(dy, qry, dz * qrz));
+            const float rinv3 = rinv * rinv2;
+            const float rinv5 = rinv3 * rinv2;
+            const float q5 = qq * rinv5;
+            // phi = -(M/r - tr/(2 r^3) + 3 q/(2 r^5))
+            ph[k] = fmaf(c0.w, rinv, ph[k]);
+            ph[k] = fmaf(c2.z, rinv3, ph[k]);
+            ph[k] = fmaf(1.5f, q5, ph[k]);
+            // a = dr (M/r^3 - 3 tr/(2 r^5) + 15 q/(2 r^7)) - 3 Q dr / r^5
+            float f = fmaf(7.5f, q5 * rinv2, c2.w * rinv5);
+            f = fmaf(c0.w, rinv3, f);
+            const float g = -3.0f * rinv5;
+            ax[k] = fmaf(dx, f, ax[k]); ax[k] = fmaf(g, qrx, ax[k]);
+            ay[k] = fmaf(dy, f, ay[k]); ay[k] = fmaf(g, qry, ay[k]);
+            az[k] = fmaf(dz, f, az[k]); az[k] = fmaf(g, qrz, az[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+        s.ax[k] += (double)ax[k]; s.ay[k] += (double)ay[k]; s.az[k] += (double)az[k]; s.ph[k] += (double)ph[k];
+    }
+    __syncwarp();
+}
+
+// Walk one chunk (<= 32 NS sinks) of group g.  Returns false on stack overflow.
+template <int NS, bool kZeroEps>
+__device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int lane, uint32_t sink_first, uint32_t ns,
+                                           const float (&bmin)[3], const float (&bmax)[3]) {
+    const uint32_t lt = (1u << lane) - 1u;
+    Sinks<NS> s;
+    uint32_t sidx[NS];
+    float smass[NS];
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+        const uint32_t off = lane + 32u * k;
+        sidx[k] = __ldg(&a.active_list[sink_first + (off < ns ? off : 0u)]);
+        const float4 p = __ldg(&a.pos[sidx[k]]);
+        s.x[k] = p.x; s.y[k] = p.y; s.z[k] = p.z;
+        smass[k] = p.w;
+        s.ax[k] = s.ay[k] = s.az[k] = s.ph[k] = 0.0;
+    }
+    uint32_t pc_r = 0, pc_w = 0, pp_r = 0, pp_w = 0;
+    uint32_t npc = 0, npp = 0;
+    int sp = 1;
+    if (lane == 0) S.stack[0] = 0u;  // the root alone: first = 0, n = 1
+    bool ok = true;
+    while (sp > 0) {
+        __syncwarp();
+        // ---- pop as many runs as fit into 32 lanes ----
+        const int navail = min(sp, 32);
+        uint32_t e = 0;
+        int cnt = 0;
+        if (lane < navail) {
+            e = S.stack[sp - 1 - lane];
+            cnt = (int)(e & 7u) + 1;
+        }
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += y;
+        }
+        const bool take = (lane < navail) && (incl <= 32);
+        const int k_taken = __popc(__ballot_sync(0xFFFFFFFFu, take));
+        const int total = __shfl_sync(0xFFFFFFFFu, incl, k_taken - 1);
+        sp -= k_taken;
+        const uint32_t startbits = __reduce_or_sync(0xFFFFFFFFu, take ? (1u << (incl - cnt)) : 0u);
+        const int j = __popc(startbits & (0xFFFFFFFFu >> (31 - lane))) - 1;
+        const uint32_t ej = __shfl_sync(0xFFFFFFFFu, e, j);
+        const int exj = __shfl_sync(0xFFFFFFFFu, incl - cnt, j);
+        const bool valid = lane < total;
+        const uint32_t cell = (ej >> 3) + (uint32_t)(lane - exj);
+        // ---- opening test (R9), every operation rounded once, in this order ----
+        bool accept = false, leaf = false;
+        uint32_t link_first = 0, info = 0;
+        if (valid) {
+            const float4* m = reinterpret_cast<const float4*>(a.mac + cell);
+            const float4 m0 = __ldg(m);
+            const float4 m1 = __ldg(m + 1);
+            const float dx = fmaxf(0.0f, fmaxf(__fsub_rn(bmin[0], m0.x), __fsub_rn(m0.x, bmax[0])));
+            const float dy = fmaxf(0.0f, fmaxf(__fsub_rn(bmin[1], m0.y), __fsub_rn(m0.y, bmax[1])));
+            const float dz = fmaxf(0.0f, fmaxf(__fsub_rn(bmin[2], m0.z), __fsub_rn(m0.z, bmax[2])));
+            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            const float rc = __fmaf_rn(m1.y, a.inv_theta, m1.x);
+            const float rc2 = __fmul_rn(rc, rc);
+            accept = d2 > rc2;
+            link_first = __float_as_uint(m1.z);
+            info = __float_as_uint(m1.w);
+            leaf = (info & kLeafBit) != 0u;
+        }
+        // ---- rejected internal cells: push their child runs ----
+        const bool open = valid && !accept && !leaf;
+        const uint32_t om = __ballot_sync(0xFFFFFFFFu, open);
+        if (open) {
+            const int pos = sp + __popc(om & lt);
+            if (pos < kWalkStack) S.stack[pos] = (link_first << 3) | (info - 1u);
+        }
+        sp += __popc(om);
+        if (sp > kWalkStack) { ok = false; break; }
+        // ---- accepted cells ----
+        const bool acc = valid && accept;
+        const uint32_t am = __ballot_sync(0xFFFFFFFFu, acc);
+        if (acc) S.pc_ids[(pc_w + __popc(am & lt)) & 63u] = cell;
+        pc_w += __popc(am);
+        npc += __popc(am);
+        __syncwarp();
+        if (pc_w - pc_r >= 32u) {
+            eval_pc<NS>(S, a, pc_r, 32, lane, s);
+            pc_r += 32u;
+        }
+        // ---- rejected leaves: expand into particles ----
+        const bool oleaf = valid && !accept && leaf;
+        const uint32_t lm = __ballot_sync(0xFFFFFFFFu, oleaf);
+        if (lm) {
+            const uint32_t lc = oleaf ? (info & ~kLeafBit) : 0u;
+            uint32_t lincl = lc;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, lincl, o);
+                if (lane >= o) lincl += y;
+            }
+            const int nl = __popc(lm);
+            const uint32_t T = __shfl_sync(0xFFFFFFFFu, lincl, 31);
+            if (oleaf) {
+                const int r = __popc(lm & lt);
+                S.leaf_first[r] = link_first;
+                S.leaf_pref[r] = lincl - lc;
+            }
+            __syncwarp();
+            npp += T;
+            for (uint32_t base = 0; base < T; base += 32u) {
+                const uint32_t t = base + lane;
+                if (t < T) {
+                    int lo = 0, hi = nl - 1;  // largest r with leaf_pref[r] <= t
+                    while (lo < hi) {
+                        const int mid = (lo + hi + 1) >> 1;
+                        if (S.leaf_pref[mid] <= t) lo = mid; else hi = mid - 1;
+                    }
+                    S.pp[(pp_w + lane) & 63u] = __ldg(&a.pos[S.leaf_first[lo] + (t - S.leaf_pref[lo])]);
+                }
+                pp_w += min(32u, T - base);
+                __syncwarp();
+                if (pp_w - pp_r >= 32u) {
+                    eval_pp<NS, kZeroEps>(S, pp_r, 32, a.eps2, s);
+                    pp_r += 32u;
+                }
+            }
+        }
+    }
+    if (!ok) return false;
+    __syncwarp();
+    if (pc_w != pc_r) eval_pc<NS>(S, a, pc_r, (int)(pc_w - pc_r), lane, s);
+    if (pp_w != pp_r) eval_pp<NS, kZeroEps>(S, pp_r, (int)(pp_w - pp_r), a.eps2, s);
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+        if (lane + 32u * k < ns) {
+            double ph = s.ph[k];
+            if (!kZeroEps) ph -= (double)(smass[k] * rsqrt_fast(a.eps2));  // the self term, bit for bit as it was added
+            const uint32_t dst = __ldg(&a.perm[sidx[k]]);
+            a.out[dst] = make_float4((float)s.ax[k], (float)s.ay[k], (float)s.az[k], (float)(-ph));
+            a.n_pp[dst] = npp - 1u;
+            a.n_pc[dst] = npc;
+        }
+    }
+    if (lane == 0) {
+        atomicAdd(&a.ctl->sum_pp, (unsigned long long)ns * (npp - 1u));
+        atomicAdd(&a.ctl->sum_pc, (unsigned long long)ns * npc);
+    }
+    return true;
+}
+
+template <bool kZeroEps>
+__global__ void __launch_bounds__(kWalkWarps * 32) k_walk(WalkArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[w];
+    const uint32_t n_groups = a.ctl->n_groups;
+    for (;;) {
+        uint32_t g = 0;
+        if (lane == 0) g = atomicAdd(&a.ctl->walk_ticket, 1u);
+        g = __shfl_sync(0xFFFFFFFFu, g, 0);
+        if (g >= n_groups) break;
+        const uint32_t gf = __ldg(&a.g_first[g]), gc = __ldg(&a.g_count[g]);
+        float bmin[3], bmax[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            bmin[k] = __ldg(&a.g_bmin[3 * g + k]);
+            bmax[k] = __ldg(&a.g_bmax[3 * g + k]);
+        }
+        // a group larger than 64 (only a level-30 leaf of coincident keys, or nleaf > ncrit) is walked in chunks
+        // of 64 sinks that all use the group's box, hence the same lists
+        for (uint32_t c0 = 0; c0 < gc; c0 += 64u) {
+            const uint32_t ns = min(64u, gc - c0);
+            bool ok;
+            if (ns > 32u) ok = walk_chunk<2, kZeroEps>(S, a, lane, gf + c0, ns, bmin, bmax);
+            else ok = walk_chunk<1, kZeroEps>(S, a, lane, gf + c0, ns, bmin, bmax);
+            if (!ok && lane == 0) a.ctl->status = BONSAI_ECAPACITY;
+            __syncwarp();
+        }
+    }
+}
+
+cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
+    Buffers& b = c->b;
+    WalkArgs a;
+    a.ctl = b.ctl;
+    a.mac = b.c_mac;
+    a.quad = b.c_quad;
+    a.pos = b.sorted_pos;
+    a.perm = b.idx[c->sorted_buf];
+    a.active_list = b.active_list;
+    a.g_first = b.g_first;
+    a.g_count = b.g_count;
+    a.g_bmin = b.g_bmin;
+    a.g_bmax = b.g_bmax;
+    a.inv_theta = 1.0f / theta;  // IEEE fp32 division on the host; theta = 0 -> +inf -> nothing is accepted
+    a.eps2 = eps * eps;
+    a.out = acc_pot_out;
+    a.n_pp = b.n_pp;
+    a.n_pc = b.n_pc;
+    const size_t smem = walk_smem_bytes(c->prm.nleaf);
+    static bool attr_set = false;
+    static int blocks_per_sm[2] = {1, 1};
+    cudaError_t e;
+    if (!attr_set) {
+        if ((e = cudaFuncSetAttribute(k_walk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(k_walk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm[0], k_walk<false>, kWalkWarps * 32, smem)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm[1], k_walk<true>, kWalkWarps * 32, smem)) != cudaSuccess) return e;
+        attr_set = true;
+    }
+    // reset the ticket and the interaction totals (adjacent fields of the control block)
+    if ((e = cudaMemsetAsync(&b.ctl->walk_ticket, 0, sizeof(uint32_t), c->stream)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&b.ctl->sum_pp, 0, 2 * sizeof(unsigned long long), c->stream)) != cudaSuccess) return e;
+    const bool zero = (a.eps2 == 0.0f);
+    const int grid = c->num_sms * max(1, blocks_per_sm[zero ? 1 : 0]);
+    if (zero) k_walk<true><<<grid, kWalkWarps * 32, smem, c->stream>>>(a);
+    else k_walk<false><<<grid, kWalkWarps * 32, smem, c->stream>>>(a);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+}  // namespace bonsai
