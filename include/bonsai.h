@@ -101,6 +101,14 @@ int bonsai_compute_multipoles(bonsai_ctx* ctx);
  * Per-particle interaction counts are kept for bonsai_get_counts().  EINVAL, ESTATE before multipoles. */
 int bonsai_walk(bonsai_ctx* ctx, float theta, float eps, const uint8_t* active_mask_dev, float* acc_pot_dev_out);
 
+/* One full force step for a caller whose particles live in HOST memory (the end-to-end path of bench.py):
+ * copies pos_mass_host (float4[n]; pinned memory recommended) to a staging buffer in the workspace, runs
+ * bonsai_load .. bonsai_walk exactly as above, copies acc_pot (float4[n], load order) back and WAITS for the
+ * stream.  active_mask_host: host u8[n] or NULL; with a mask, acc_pot_host_out is also read (entries of inactive
+ * particles are returned unchanged).  Returns what bonsai_sync() returns, or EINVAL / ECUDA. */
+int bonsai_step_host(bonsai_ctx* ctx, const float* pos_mass_host, uint32_t n, float theta, float eps,
+                     const uint8_t* active_mask_host, float* acc_pot_host_out);
+
 /* Release the context (host memory only; the workspace belongs to the caller).  NULL is allowed. */
 void bonsai_destroy(bonsai_ctx* ctx);
 

@@ -24,7 +24,7 @@ STAGES = ("bbox", "keys", "sort", "reorder", "build", "groups", "multipoles", "w
 # every symbol include/bonsai.h declares (tests check the library exports exactly these)
 SYMBOLS = (
     "bonsai_workspace_bytes", "bonsai_create", "bonsai_load", "bonsai_build_tree",
-    "bonsai_compute_multipoles", "bonsai_walk", "bonsai_destroy", "bonsai_sync", "bonsai_get_box",
+    "bonsai_compute_multipoles", "bonsai_walk", "bonsai_step_host", "bonsai_destroy", "bonsai_sync", "bonsai_get_box",
     "bonsai_get_keys", "bonsai_get_perm", "bonsai_get_sorted_pos", "bonsai_get_cells", "bonsai_get_groups",
     "bonsai_get_counts", "bonsai_get_interaction_totals", "bonsai_set_timing", "bonsai_get_stage_ms",
     "bonsai_get_launch_count", "bonsai_strerror",
@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
     L.bonsai_build_tree.argtypes = [vp]
     L.bonsai_compute_multipoles.argtypes = [vp]
     L.bonsai_walk.argtypes = [vp, f32, f32, vp, vp]
+    L.bonsai_step_host.argtypes = [vp, vp, u32, f32, f32, vp, vp]
     L.bonsai_destroy.argtypes = [vp]
     L.bonsai_destroy.restype = None
     L.bonsai_sync.argtypes = [vp]
@@ -211,6 +212,24 @@ class Bonsai:
         self.build_tree()
         self.compute_multipoles()
         return self.walk(theta, eps, active_mask, out)
+
+    def step_host(self, pos_mass_host: torch.Tensor, theta: float, eps: float,
+                  active_mask_host: torch.Tensor | None = None, out_host: torch.Tensor | None = None) -> torch.Tensor:
+        """bonsai_step_host: HOST tensors in (float32[n,4], ideally pinned), HOST float32[n,4] out; blocking."""
+        assert not pos_mass_host.is_cuda and pos_mass_host.dtype == torch.float32 and pos_mass_host.is_contiguous()
+        n = pos_mass_host.shape[0]
+        if out_host is None:
+            out_host = torch.zeros((n, 4), dtype=torch.float32).pin_memory()
+        assert not out_host.is_cuda and out_host.dtype == torch.float32 and out_host.is_contiguous()
+        mptr = None
+        if active_mask_host is not None:
+            assert not active_mask_host.is_cuda and active_mask_host.dtype == torch.uint8
+            mptr = active_mask_host.data_ptr()
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_step_host(self._h, pos_mass_host.data_ptr(), n, float(theta), float(eps), mptr,
+                                            out_host.data_ptr()), "bonsai_step_host")
+        self.n = n
+        return out_host
 
     def sync(self) -> None:
         _check(self._L.bonsai_sync(self._h), "bonsai_sync")

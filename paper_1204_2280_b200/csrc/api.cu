@@ -93,6 +93,9 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     t.scan_tmp = cv.take<uint32_t>((size_t)div_up(n + 1, 2048) + 2);
     t.n_pp = cv.take<uint32_t>(n);
     t.n_pc = cv.take<uint32_t>(n);
+    t.host_in = cv.take<float4>(n);
+    t.host_out = cv.take<float4>(n);
+    t.host_mask = cv.take<uint8_t>(n);
     if (b) *b = t;
     return (cv.off + kAlign - 1) / kAlign * kAlign;
 }
@@ -216,6 +219,28 @@ int bonsai_walk(bonsai_ctx* h, float theta, float eps, const uint8_t* active_mas
     { StageTimer t(c, 7); BONSAI_TRY(stage_walk(c, theta, eps, reinterpret_cast<float4*>(acc_pot_dev_out))); }
     c->state = 4;
     return BONSAI_OK;
+}
+
+int bonsai_step_host(bonsai_ctx* h, const float* pos_mass_host, uint32_t n, float theta, float eps,
+                     const uint8_t* active_mask_host, float* acc_pot_host_out) {
+    if (!h || !pos_mass_host || !acc_pot_host_out) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    if (n == 0 || n > c->n_max) return BONSAI_EINVAL;
+    Buffers& b = c->b;
+    BONSAI_TRY(cudaMemcpyAsync(b.host_in, pos_mass_host, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    if (active_mask_host) {
+        BONSAI_TRY(cudaMemcpyAsync(b.host_mask, active_mask_host, (size_t)n, cudaMemcpyHostToDevice, c->stream));
+        // entries of inactive particles are defined to stay untouched: start from the caller's values
+        BONSAI_TRY(cudaMemcpyAsync(b.host_out, acc_pot_host_out, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    }
+    int rc;
+    if ((rc = bonsai_load(h, reinterpret_cast<const float*>(b.host_in), n)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_walk(h, theta, eps, active_mask_host ? b.host_mask : nullptr,
+                          reinterpret_cast<float*>(b.host_out))) != BONSAI_OK) return rc;
+    BONSAI_TRY(cudaMemcpyAsync(acc_pot_host_out, b.host_out, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
+    return bonsai_sync(h);
 }
 
 void bonsai_destroy(bonsai_ctx* h) {

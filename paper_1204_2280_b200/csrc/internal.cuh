@@ -96,6 +96,9 @@ struct Buffers {
     uint32_t* scan_tmp;        // block sums of the device-wide scan
     // walk
     uint32_t *n_pp, *n_pc;     // [n] load order
+    // staging of bonsai_step_host
+    float4 *host_in, *host_out;
+    uint8_t* host_mask;
 };
 
 struct Ctx {
