@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the headline metric of BASELINE.json:
+
+    "Plummer 4M theta=0.75 particles/s per full step; walk flop/s vs FP32 peak"
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one pass of the whole hot path (bbox, keys, sort, reorder, build, groups,
+multipoles, walk) over the seeded Plummer sphere of BASELINE.json configs[3] (N = 2^22, eps = 0.00125,
+theta = 0.75), all particles active.  `value` = particles / device time of a step with the particles already
+resident in HBM; `e2e` = the same through bonsai_step_host() with HOST buffers (H2D of the particles and D2H of
+acc/pot inside the timed region).  The path does not shard ("replicas only"): with
+--gpus N > 1 every rank runs the same step on its own replica, no collective on the data path, and `value` is
+the sum over ranks of N / (max over ranks of the time).
+
+--impl reference times the CPU oracle (oracle/, single thread, fp64), as it stands, on a bounded sample of the
+same workload; it needs no GPU.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "particles_per_second_full_step"
+UNIT = "particles/s"
+FLOP_PP, FLOP_PC = 20, 63          # DESIGN.md R20: FMA = 2 flop, rsqrt = 1
+FP32_LANES_PER_SM = 128            # B200 (sm_100): 4 SMSPs x 32 FP32 lanes, 2 flop per lane per clock (FMA)
+L2_FLUSH_BYTES = 256 << 20         # > 126 MB L2
+
+
+def _workload(name: str):
+    from paper_1204_2280_b200 import workloads as W
+    cfg = W.CONFIGS[name]
+    return W, cfg["n"], cfg["theta"], cfg["eps"]
+
+
+# ------------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of the default run, and --impl reference)
+# ------------------------------------------------------------------------------------------------------
+def oracle_step_sample(pm, theta, eps, ncrit, group_mode, walk_budget_s):
+    """The oracle's full step, its walk restricted to an evenly spaced sample of the groups.
+
+    All stages before the walk run in full; the walk (>= 98 % of the oracle's time) is first probed on 64
+    groups, then timed on every `stride`-th group with `stride` the smallest power of two that keeps it within
+    `walk_budget_s`, and scaled by n_groups / n_sampled (the groups are evenly spaced along the Morton curve).
+    Returns (estimated seconds of one full step, description of the sample).
+    """
+    import oracle as O
+    t0 = time.perf_counter()
+    s = O.build(pm, 16, ncrit, group_mode)
+    t_build = time.perf_counter() - t0
+    ng = s.groups.n_groups
+    probe = np.unique(np.linspace(0, ng - 1, min(ng, 64)).astype(np.uint32))
+    t0 = time.perf_counter()
+    O.walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, probe)
+    per_group = (time.perf_counter() - t0) / len(probe)
+    stride = 1
+    while per_group * ng / stride > walk_budget_s and stride < ng:
+        stride *= 2
+    sel = np.arange(0, ng, stride, dtype=np.uint32)
+    t0 = time.perf_counter()
+    O.walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
+    t_walk = time.perf_counter() - t0
+    est = t_build + t_walk * (ng / len(sel))
+    what = (f"all pre-walk stages on all {pm.shape[0]} particles ({t_build:.2f} s) + walk of {len(sel)} of {ng} "
+            f"groups (every {stride}th, {t_walk:.2f} s) scaled by {ng}/{len(sel)}")
+    return est, what
+
+
+def cpu_baseline(pm, theta, eps, ncrit, group_mode, budget_s=15.0):
+    est, what = oracle_step_sample(pm, theta, eps, ncrit, group_mode, budget_s)
+    return {"value": pm.shape[0] / est, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
+            "est_full_step_s": est}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    W, n, theta, eps = _workload(args.workload)
+    pm = W.plummer(n)
+    # each step: the full pre-walk stages + a walk sample bounded to ~8 s
+    for _ in range(min(args.warmup, 1)):
+        oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, 2.0)
+    ests, what = [], ""
+    for _ in range(args.steps):
+        est, what = oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, 8.0)
+        ests.append(est)
+    est = float(np.mean(ests))
+    value = n / est
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": est * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "n": n, "theta": theta, "eps": eps, "nleaf": 16,
+                   "ncrit": args.ncrit, "group_mode": args.group_mode},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU, sampled every 50 ms while running."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.thread = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append((time.perf_counter(), ln.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for t, ln in self.rows:
+            if not (t0 - 0.05 <= t <= t1 + 0.15):
+                continue
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- libbonsai has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_1204_2280_b200 import Bonsai
+    W, n, theta, eps = _workload(args.workload)
+    pm = W.plummer(n)
+    peaks = {}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            peaks = json.load(f)
+    except OSError:
+        pass
+
+    stream = torch.cuda.Stream(dev)
+    b = Bonsai(n, ncrit=args.ncrit, group_mode=args.group_mode, device=dev, stream=stream)
+    b.set_timing(True)
+    d_pm = torch.from_numpy(pm).to(dev)
+    d_out = torch.zeros((n, 4), dtype=torch.float32, device=dev)
+    h_pm = torch.from_numpy(pm).pin_memory()
+    h_out = torch.zeros((n, 4), dtype=torch.float32).pin_memory()
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def flush_l2():
+        with torch.cuda.stream(stream):
+            flush.fill_(1)
+
+    def one_step():
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        flush_l2()
+        e0.record(stream)
+        b.step(d_pm, theta, eps, None, d_out)
+        e1.record(stream)
+        return e0, e1
+
+    def one_step_host():
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        flush_l2()
+        e0.record(stream)
+        b.step_host(h_pm, theta, eps, None, h_out)   # blocking: returns after the D2H copy
+        e1.record(stream)
+        return e0, e1
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None   # started early: nvidia-smi takes a moment to come up
+    for _ in range(args.warmup):
+        one_step()
+        b.sync()
+    # ---- timed region: exactly K steps, device-resident inputs ----
+    barrier()
+    launches0 = b.launch_count()
+    t_wall0 = time.perf_counter()
+    step_ms, stage_ms = [], []
+    for _ in range(args.steps):
+        e0, e1 = one_step()
+        b.sync()
+        step_ms.append(e0.elapsed_time(e1))
+        stage_ms.append(b.stage_ms())
+    barrier()
+    t_wall1 = time.perf_counter()
+    launches = b.launch_count() - launches0
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    sum_pp, sum_pc = b.interaction_totals()
+    total_ms = float(sum(step_ms))
+
+    # ---- end to end through the host-buffer call ----
+    for _ in range(min(args.warmup, 2)):
+        one_step_host()
+    barrier()
+    e2e_ms = []
+    for _ in range(args.steps):
+        e0, e1 = one_step_host()
+        torch.cuda.synchronize(dev)
+        e2e_ms.append(e0.elapsed_time(e1))
+    barrier()
+    e2e_total_ms = float(sum(e2e_ms))
+
+    if world > 1:
+        t = torch.tensor([total_ms, e2e_total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_total_ms = float(t[0]), float(t[1])
+
+    if rank == 0:
+        ms_per_step = total_ms / args.steps
+        value = world * n * args.steps / (total_ms * 1e-3)
+        e2e_value = world * n * args.steps / (e2e_total_ms * 1e-3)
+        st = {k: float(np.mean([s[k] for s in stage_ms])) for k in stage_ms[0]}
+        walk_ms = st["walk"]
+        flop = FLOP_PP * sum_pp + FLOP_PC * sum_pc
+        sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+        n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_tf = n_sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+        achieved_tf = flop / (walk_ms * 1e-3) / 1e12
+        hbm = peaks.get("hbm_gbs", 6650.0)
+        hbm_src = "measured" if "hbm_gbs" in peaks else "fallback"
+        # algorithmic bytes per particle of the HBM-bound stages
+        alg_bytes = {"bbox": 16, "keys": 32, "sort": 12 + 9 * 32, "reorder": 36, "groups": 16 + 24 / args.ncrit}
+        stages = {}
+        for k, v in st.items():
+            ent = {"ms": v, "share": v / sum(st.values())}
+            if k in alg_bytes and v > 0:
+                gbs = alg_bytes[k] * n / (v * 1e-3) / 1e9
+                ent.update({"alg_gbs": gbs, "hbm_frac": gbs / hbm})
+            stages[k] = ent
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "n": n, "theta": theta, "eps": eps, "nleaf": 16,
+                       "ncrit": args.ncrit, "group_mode": args.group_mode, "parallelism": "replicas only",
+                       "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB fill, outside the event pair)",
+                       "paper_context": "GTX480: > 2.8e6 particles/s (PAPER.md:14), other hardware"},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_total_ms / args.steps,
+                    "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n},
+            "gpu_launches": int(launches),
+            "roofline": {"kernel": "k_walk", "bound": "alu", "achieved": achieved_tf, "peak": peak_tf,
+                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+                         "peak_source": f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x "
+                                        f"{sm_max:.0f} MHz (clocks.max.sm); no fp32 entry in MEASURED_PEAKS.json",
+                         "flop_convention": "20 per p-p, 63 per p-c (FMA = 2, rsqrt = 1)",
+                         "walk_ms": walk_ms, "walk_share_of_step": walk_ms / sum(st.values()),
+                         "interactions_per_s": (sum_pp + sum_pc) / (walk_ms * 1e-3),
+                         "pp_per_particle": sum_pp / n, "pc_per_particle": sum_pc / n,
+                         "hbm_peak_gbs": hbm, "hbm_peak_source": hbm_src},
+            "stages": stages,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(pm, theta, eps, args.ncrit, args.group_mode)
+        print(json.dumps(line), flush=True)
+    b.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--workload", default="plummer_4m")
+    ap.add_argument("--ncrit", type=int, default=64)
+    ap.add_argument("--group-mode", dest="group_mode", type=int, default=1)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 3)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
