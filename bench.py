@@ -48,17 +48,17 @@ def _workload(name: str):
 # ------------------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline of the default run, and --impl reference)
 # ------------------------------------------------------------------------------------------------------
-def oracle_step_sample(pm, theta, eps, ncrit, group_mode, walk_budget_s):
+def oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, walk_budget_s):
     """The oracle's full step, its walk restricted to an evenly spaced sample of the groups.
 
     All stages before the walk run in full; the walk (>= 98 % of the oracle's time) is first probed on 64
     groups, then timed on every `stride`-th group with `stride` the smallest power of two that keeps it within
-    `walk_budget_s`, and scaled by n_groups / n_sampled (the groups are evenly spaced along the Morton curve).
+    `walk_budget_s`, and scaled by n_particles / n_sinks_sampled (the groups are evenly spaced along the Morton curve).
     Returns (estimated seconds of one full step, description of the sample).
     """
     import oracle as O
     t0 = time.perf_counter()
-    s = O.build(pm, 16, ncrit, group_mode)
+    s = O.build(pm, 16, ncrit, group_mode, None, None, group_cell)
     t_build = time.perf_counter() - t0
     ng = s.groups.n_groups
     probe = np.unique(np.linspace(0, ng - 1, min(ng, 64)).astype(np.uint32))
@@ -72,14 +72,15 @@ def oracle_step_sample(pm, theta, eps, ncrit, group_mode, walk_budget_s):
     t0 = time.perf_counter()
     O.walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
     t_walk = time.perf_counter() - t0
-    est = t_build + t_walk * (ng / len(sel))
+    n_sinks = int(s.groups.count[sel].sum())
+    est = t_build + t_walk * (s.groups.n_active / n_sinks)
     what = (f"all pre-walk stages on all {pm.shape[0]} particles ({t_build:.2f} s) + walk of {len(sel)} of {ng} "
-            f"groups (every {stride}th, {t_walk:.2f} s) scaled by {ng}/{len(sel)}")
+            f"groups (every {stride}th, {n_sinks} sinks, {t_walk:.2f} s) scaled by {s.groups.n_active}/{n_sinks}")
     return est, what
 
 
-def cpu_baseline(pm, theta, eps, ncrit, group_mode, budget_s=15.0):
-    est, what = oracle_step_sample(pm, theta, eps, ncrit, group_mode, budget_s)
+def cpu_baseline(pm, theta, eps, ncrit, group_mode, group_cell, budget_s=15.0):
+    est, what = oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, budget_s)
     return {"value": pm.shape[0] / est, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
             "est_full_step_s": est}
 
@@ -92,10 +93,10 @@ def run_reference(args):
     pm = W.plummer(n)
     # each step: the full pre-walk stages + a walk sample bounded to ~8 s
     for _ in range(min(args.warmup, 1)):
-        oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, 2.0)
+        oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 2.0)
     ests, what = [], ""
     for _ in range(args.steps):
-        est, what = oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, 8.0)
+        est, what = oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 8.0)
         ests.append(est)
     est = float(np.mean(ests))
     value = n / est
@@ -104,7 +105,7 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": est * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "n": n, "theta": theta, "eps": eps, "nleaf": 16,
-                   "ncrit": args.ncrit, "group_mode": args.group_mode},
+                   "ncrit": args.ncrit, "group_mode": args.group_mode, "group_cell": args.group_cell},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -195,7 +196,7 @@ def run_ours(args):
         pass
 
     stream = torch.cuda.Stream(dev)
-    b = Bonsai(n, ncrit=args.ncrit, group_mode=args.group_mode, device=dev, stream=stream)
+    b = Bonsai(n, ncrit=args.ncrit, group_mode=args.group_mode, group_cell=args.group_cell, device=dev, stream=stream)
     b.set_timing(True)
     d_pm = torch.from_numpy(pm).to(dev)
     d_out = torch.zeros((n, 4), dtype=torch.float32, device=dev)
@@ -294,7 +295,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "n": n, "theta": theta, "eps": eps, "nleaf": 16,
-                       "ncrit": args.ncrit, "group_mode": args.group_mode, "parallelism": "replicas only",
+                       "ncrit": args.ncrit, "group_mode": args.group_mode, "group_cell": args.group_cell, "parallelism": "replicas only",
                        "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB fill, outside the event pair)",
                        "paper_context": "GTX480: > 2.8e6 particles/s (PAPER.md:14), other hardware"},
             "clocks": clocks,
@@ -313,7 +314,7 @@ def run_ours(args):
             "stages": stages,
         }
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(pm, theta, eps, args.ncrit, args.group_mode)
+            line["cpu_baseline"] = cpu_baseline(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell)
         print(json.dumps(line), flush=True)
     b.close()
     if world > 1:
@@ -330,7 +331,8 @@ def main():
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--workload", default="plummer_4m")
     ap.add_argument("--ncrit", type=int, default=64)
-    ap.add_argument("--group-mode", dest="group_mode", type=int, default=1)
+    ap.add_argument("--group-mode", dest="group_mode", type=int, default=2)
+    ap.add_argument("--group-cell", dest="group_cell", type=int, default=1024)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

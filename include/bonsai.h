@@ -50,16 +50,20 @@ typedef struct bonsai_ctx bonsai_ctx; /* opaque, host memory, owned by the libra
 typedef struct {
     uint32_t nleaf;      /* [16] a cell with <= nleaf particles is a leaf (R7); 1..64                        */
     uint32_t ncrit;      /* [64] maximum particles per walk group (R13); 1..64                               */
-    uint32_t group_mode; /* 0 = tree-cell groups, 1 = consecutive sorted chunks [1] (R13).  NOTE: because 0 is
-                            a legal value, group_mode is only defaulted when params == NULL.                   */
-    uint32_t cap_cells;  /* [n_max + 64] capacity of the cell arrays                                         */
+    uint32_t group_mode; /* 0 = tree-cell groups, 1 = consecutive sorted chunks, 2 = chunks of ncrit inside the
+                            cells with <= group_cell particles [2] (R13).  NOTE: because 0 is a legal value,
+                            group_mode is only defaulted when params == NULL.                                 */
+    uint32_t cap_cells;  /* [2 n_max + 256] capacity of the cell arrays                                      */
+    uint32_t group_cell; /* [1024] mode 2: a group never crosses the boundary of a cell holding more than
+                            group_cell particles (the containers are the cells with count <= group_cell whose
+                            parent has more); >= ncrit                                                        */
 } bonsai_params;
 
 /* Bytes of device workspace bonsai_create() needs for up to n_max particles (0 on bad arguments). */
 size_t bonsai_workspace_bytes(uint32_t n_max, const bonsai_params* params);
 
 /* Create a context for up to n_max particles.
- *   params         host pointer or NULL (all defaults, group_mode = 1)
+ *   params         host pointer or NULL (all defaults, group_mode = 2)
  *   workspace_dev  device pointer, 256-byte aligned, >= bonsai_workspace_bytes() bytes, caller-owned
  *   cuda_stream    a cudaStream_t (NULL = the legacy default stream)
  *   out            host pointer receiving the context

@@ -117,7 +117,7 @@ class Groups:
     bmax: np.ndarray
 
 
-def groups(mode, ncrit, sorted_pos_mass, t: Tree, active_sorted=None):
+def groups(mode, ncrit, sorted_pos_mass, t: Tree, active_sorted=None, group_cell=1024):
     spm = _f32(sorted_pos_mass)
     n = spm.shape[0]
     act = None if active_sorted is None else np.ascontiguousarray(active_sorted, dtype=np.uint8)
@@ -127,7 +127,7 @@ def groups(mode, ncrit, sorted_pos_mass, t: Tree, active_sorted=None):
     bmin = np.zeros((n, 3), np.float32)
     bmax = np.zeros((n, 3), np.float32)
     na = C.c_uint32(0)
-    ng = lib().oracle_groups(C.c_uint32(mode), C.c_uint32(ncrit), C.c_uint32(n), _p(spm, C.c_float),
+    ng = lib().oracle_groups(C.c_uint32(mode), C.c_uint32(ncrit), C.c_uint32(group_cell), C.c_uint32(n), _p(spm, C.c_float),
                              C.c_uint32(t.n_cells), _p(t.first, C.c_uint32), _p(t.count, C.c_uint32),
                              _p(t.first_child, C.c_uint32), _p(t.n_child, C.c_uint32),
                              _p(act, C.c_uint8), _p(active_list, C.c_uint32), C.byref(na),
@@ -231,7 +231,7 @@ class Step:
         return out
 
 
-def build(pos_mass, nleaf=16, ncrit=64, group_mode=1, active_mask=None, cap_cells=None) -> Step:
+def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cells=None, group_cell=1024) -> Step:
     """O1..O6: box, keys, sort, reorder, tree, groups, multipoles.  active_mask is in LOAD order."""
     pm = _f32(pos_mass)
     lo, side = box(pm)
@@ -240,12 +240,13 @@ def build(pos_mass, nleaf=16, ncrit=64, group_mode=1, active_mask=None, cap_cell
     spm, sk = reorder(pm, k, perm)
     t = tree(sk, nleaf, cap_cells)
     act_sorted = None if active_mask is None else np.ascontiguousarray(active_mask, np.uint8)[perm]
-    g = groups(group_mode, ncrit, spm, t, act_sorted)
+    g = groups(group_mode, ncrit, spm, t, act_sorted, group_cell)
     multipoles(spm, sk, lo, side, t)
     return Step(lo, side, k, perm, spm, sk, t, g)
 
 
-def full_step(pos_mass, theta, eps, nleaf=16, ncrit=64, group_mode=1, active_mask=None, sel=None) -> Step:
-    s = build(pos_mass, nleaf, ncrit, group_mode, active_mask)
+def full_step(pos_mass, theta, eps, nleaf=16, ncrit=64, group_mode=2, active_mask=None, sel=None,
+              group_cell=1024) -> Step:
+    s = build(pos_mass, nleaf, ncrit, group_mode, active_mask, None, group_cell)
     s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
     return s

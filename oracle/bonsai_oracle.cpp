@@ -220,10 +220,15 @@ uint32_t oracle_tree(const uint32_t* sorted_keys, uint32_t n, uint32_t nleaf, ui
 //       n <= ncrit; a level-30 leaf may exceed ncrit), in key order; a group keeps only its active
 //       members and is dropped if none remain.
 //   mode 1 (sorted-chunk): consecutive runs of ncrit active particles (last one shorter).
+//   mode 2 (cell-chunk): the "container" cells are the mode-0 cells at threshold group_cell (count <=
+//       group_cell, parent count > group_cell; childless cells always qualify); the active members of each
+//       container, in sorted order, are cut into consecutive runs of ncrit (last one shorter).  A group
+//       therefore never straddles the boundary of a cell holding more than group_cell particles.
+//       group_cell = ncrit gives mode 0 for every cell with <= ncrit particles, group_cell >= n gives mode 1.
 // bmin/bmax: exact fp32 per-axis min/max over the group's members (3 floats per group each).
 // Returns n_groups; *n_active_out = number of active particles.
 // -------------------------------------------------------------------------------------
-uint32_t oracle_groups(uint32_t mode, uint32_t ncrit, uint32_t n, const float* sorted_pos_mass,
+uint32_t oracle_groups(uint32_t mode, uint32_t ncrit, uint32_t group_cell, uint32_t n, const float* sorted_pos_mass,
                        uint32_t n_cells, const uint32_t* first, const uint32_t* count,
                        const uint32_t* first_child, const uint32_t* n_child,
                        const uint8_t* active_sorted, uint32_t* active_list, uint32_t* n_active_out,
@@ -258,10 +263,16 @@ uint32_t oracle_groups(uint32_t mode, uint32_t ncrit, uint32_t n, const float* s
         std::vector<uint32_t> stack;
         stack.push_back(0);
         (void)n_cells;
+        const uint32_t limit = (mode == 2) ? group_cell : ncrit;
         while (!stack.empty()) {
             uint32_t c = stack.back(); stack.pop_back();
-            if (count[c] <= ncrit || n_child[c] == 0) {
-                emit(rank[first[c]], rank[first[c] + count[c]] - rank[first[c]]);
+            if (count[c] <= limit || n_child[c] == 0) {
+                const uint32_t r0 = rank[first[c]], a = rank[first[c] + count[c]] - r0;
+                if (mode == 2) {
+                    for (uint32_t f = 0; f < a; f += ncrit) emit(r0 + f, std::min(ncrit, a - f));
+                } else {
+                    emit(r0, a);
+                }
             } else {
                 for (uint32_t k = n_child[c]; k-- > 0;) stack.push_back(first_child[c] + k);
             }

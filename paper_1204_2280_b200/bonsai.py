@@ -33,7 +33,7 @@ SYMBOLS = (
 
 class Params(C.Structure):
     _fields_ = [("nleaf", C.c_uint32), ("ncrit", C.c_uint32), ("group_mode", C.c_uint32),
-                ("cap_cells", C.c_uint32)]
+                ("cap_cells", C.c_uint32), ("group_cell", C.c_uint32)]
 
 
 class CellsView(C.Structure):
@@ -103,9 +103,9 @@ def _check(code: int, what: str) -> None:
         raise BonsaiError(code, what)
 
 
-def workspace_bytes(n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 1,
-                    cap_cells: int = 0) -> int:
-    p = Params(nleaf, ncrit, group_mode, cap_cells)
+def workspace_bytes(n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
+                    cap_cells: int = 0, group_cell: int = 0) -> int:
+    p = Params(nleaf, ncrit, group_mode, cap_cells, group_cell)
     return int(lib().bonsai_workspace_bytes(n_max, C.byref(p)))
 
 
@@ -147,8 +147,8 @@ class Bonsai:
     ``stream`` (default: the current torch stream at construction).
     """
 
-    def __init__(self, n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 1,
-                 cap_cells: int = 0, device: str | torch.device = "cuda:0",
+    def __init__(self, n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
+                 cap_cells: int = 0, group_cell: int = 0, device: str | torch.device = "cuda:0",
                  stream: "torch.cuda.Stream | None" = None):
         if not torch.cuda.is_available():
             raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -156,7 +156,7 @@ class Bonsai:
         self._L = lib()
         self.n_max = int(n_max)
         self.n = 0
-        self.params = Params(nleaf, ncrit, group_mode, cap_cells)
+        self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell)
         nbytes = int(self._L.bonsai_workspace_bytes(self.n_max, C.byref(self.params)))
         if nbytes == 0:
             raise BonsaiError(EINVAL, "bonsai_workspace_bytes")

@@ -30,13 +30,16 @@ struct Carver {
 
 bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out) {
     bonsai_params p;
-    p.nleaf = 16; p.ncrit = 64; p.group_mode = 1; p.cap_cells = 0;
+    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0;
     if (in) {
         if (in->nleaf) p.nleaf = in->nleaf;
         if (in->ncrit) p.ncrit = in->ncrit;
         p.group_mode = in->group_mode;
         p.cap_cells = in->cap_cells;
+        p.group_cell = in->group_cell;
     }
+    if (p.group_cell == 0) p.group_cell = 1024;
+    if (p.group_cell < p.ncrit) p.group_cell = p.ncrit;
     if (p.cap_cells == 0) {
         unsigned long long cap = 2ull * n_max + 256ull;
         if (cap >= (1ull << 29)) cap = (1ull << 29) - 1;
@@ -45,7 +48,7 @@ bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out)
     if (n_max == 0 || n_max > (1u << 30)) return false;
     if (p.nleaf < 1 || p.nleaf > (uint32_t)kMaxNleaf) return false;
     if (p.ncrit < 1 || p.ncrit > (uint32_t)kMaxNcrit) return false;
-    if (p.group_mode > 1) return false;
+    if (p.group_mode > 2) return false;
     if (p.cap_cells < 1 || p.cap_cells >= (1u << 29)) return false;  // walk stack entries pack the id into 29 bits
     *out = p;
     return true;

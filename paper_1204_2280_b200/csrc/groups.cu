@@ -6,6 +6,9 @@
 //   mode 1 (sorted chunks): group g = active particles [g ncrit, min((g+1) ncrit, n_active))
 //   mode 0 (tree cells):    the cells with count <= ncrit (or childless) whose parent has count > ncrit, in key
 //                           order, each keeping only its active members, dropped when none remain
+//   mode 2 (cell chunks):   the active members of every container cell (count <= group_cell or childless, parent
+//                           count > group_cell) are cut into consecutive runs of ncrit: no group straddles the
+//                           boundary of a big cell, which bounds the most expensive group
 //   bmin / bmax            exact fp32 per-axis min / max over the group's members
 #include "internal.cuh"
 
@@ -50,7 +53,8 @@ __global__ void __launch_bounds__(256) k_groups_chunks(const uint32_t* __restric
 }
 
 // mode 0, step 1: mark the first particle of every non-empty group cell
-__global__ void __launch_bounds__(256) k_groups_mark(const Control* __restrict__ ctl, uint32_t cap_cells, uint32_t ncrit,
+__global__ void __launch_bounds__(256) k_groups_mark(const Control* __restrict__ ctl, uint32_t cap_cells, uint32_t limit,
+                                                     uint32_t chunk,
                                                      const uint32_t* __restrict__ c_first,
                                                      const uint32_t* __restrict__ c_count,
                                                      const uint32_t* __restrict__ c_n_child,
@@ -60,12 +64,13 @@ __global__ void __launch_bounds__(256) k_groups_mark(const Control* __restrict__
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= min(ctl->n_cells, cap_cells)) return;
     const uint32_t cnt = c_count[c];
-    if (!(cnt <= ncrit || c_n_child[c] == 0)) return;
+    if (!(cnt <= limit || c_n_child[c] == 0)) return;
     const uint32_t p = c_parent[c];
-    if (p != kNone && c_count[p] <= ncrit) return;  // an ancestor already is the group
+    if (p != kNone && c_count[p] <= limit) return;  // an ancestor already is the group / container
     const uint32_t f = c_first[c];
-    if (rank[f + cnt] == rank[f]) return;            // no active member
-    g_flag[f] = 1u;
+    const uint32_t a = rank[f + cnt] - rank[f];
+    if (a == 0) return;                              // no active member
+    g_flag[f] = chunk ? (a + chunk - 1u) / chunk : 1u;  // number of groups this cell contributes
     g_cell[f] = c + 1u;
 }
 
@@ -73,8 +78,9 @@ __global__ void __launch_bounds__(256) k_groups_mark(const Control* __restrict__
 __global__ void __launch_bounds__(256) k_groups_cells(const uint32_t* __restrict__ g_index,
                                                       const uint32_t* __restrict__ g_cell, uint32_t n,
                                                       const uint32_t* __restrict__ c_count,
-                                                      const uint32_t* __restrict__ rank, uint32_t* __restrict__ g_first,
-                                                      uint32_t* __restrict__ g_count, Control* __restrict__ ctl) {
+                                                      const uint32_t* __restrict__ rank, uint32_t chunk,
+                                                      uint32_t* __restrict__ g_first, uint32_t* __restrict__ g_count,
+                                                      Control* __restrict__ ctl) {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) ctl->n_groups = g_index[n];
     if (i >= n) return;
@@ -82,8 +88,17 @@ __global__ void __launch_bounds__(256) k_groups_cells(const uint32_t* __restrict
     if (c1 == 0) return;
     const uint32_t g = g_index[i];
     const uint32_t r0 = rank[i];
-    g_first[g] = r0;
-    g_count[g] = rank[i + c_count[c1 - 1]] - r0;
+    const uint32_t a = rank[i + c_count[c1 - 1]] - r0;
+    if (chunk == 0u) {
+        g_first[g] = r0;
+        g_count[g] = a;
+    } else {
+        uint32_t k = 0;
+        for (uint32_t o = 0; o < a; o += chunk, ++k) {
+            g_first[g + k] = r0 + o;
+            g_count[g + k] = min(chunk, a - o);
+        }
+    }
 }
 
 // one warp per group (grid-stride): exact fp32 box
@@ -139,13 +154,16 @@ cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order) {
     } else {
         if ((e = cudaMemsetAsync(b.g_flag, 0, sizeof(uint32_t) * (size_t)(n + 1), c->stream)) != cudaSuccess) return e;
         if ((e = cudaMemsetAsync(b.g_cell, 0, sizeof(uint32_t) * (size_t)n, c->stream)) != cudaSuccess) return e;
-        k_groups_mark<<<div_up(c->cap_cells, 256), 256, 0, c->stream>>>(b.ctl, c->cap_cells, c->prm.ncrit, b.c_first,
+        const bool cells = (c->prm.group_mode == 0);
+        const uint32_t limit = cells ? c->prm.ncrit : c->prm.group_cell;
+        const uint32_t chunk = cells ? 0u : c->prm.ncrit;
+        k_groups_mark<<<div_up(c->cap_cells, 256), 256, 0, c->stream>>>(b.ctl, c->cap_cells, limit, chunk, b.c_first,
                                                                         b.c_count, b.c_n_child, b.c_parent, b.rank,
                                                                         b.g_flag, b.g_cell);
         c->launches += 1;
         if ((e = exclusive_scan_u32(c, b.g_flag, b.g_flag, n, b.scan_tmp)) != cudaSuccess) return e;
-        k_groups_cells<<<div_up(n, 256), 256, 0, c->stream>>>(b.g_flag, b.g_cell, n, b.c_count, b.rank, b.g_first,
-                                                              b.g_count, b.ctl);
+        k_groups_cells<<<div_up(n, 256), 256, 0, c->stream>>>(b.g_flag, b.g_cell, n, b.c_count, b.rank, chunk,
+                                                              b.g_first, b.g_count, b.ctl);
         c->launches += 1;
     }
     k_groups_box<<<c->num_sms * 8, 256, 0, c->stream>>>(b.ctl, b.g_first, b.g_count, b.active_list, b.sorted_pos,

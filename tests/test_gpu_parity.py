@@ -132,7 +132,7 @@ def run_gpu(pm, theta, eps, mask=None, **kw):
 
 
 @pytest.mark.parametrize("n", [1, 2, 15, 16, 17, 33, 100, 1000, 4097])
-@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1, 2])
 def test_small_sizes_full_step(n, mode):
     pm = W.plummer(n)
     ref = O.full_step(pm, 0.75, 0.01, group_mode=mode)
@@ -145,12 +145,13 @@ def test_small_sizes_full_step(n, mode):
         assert np.all(out == 0.0)
 
 
-@pytest.mark.parametrize("mode,ncrit", [(1, 64), (0, 64), (1, 32), (0, 32)])
-def test_config0_32k(mode, ncrit):
+@pytest.mark.parametrize("mode,ncrit,group_cell", [(2, 64, 1024), (2, 32, 1024), (2, 32, 100), (1, 64, 0), (0, 64, 0),
+                                                   (1, 32, 0), (0, 32, 0)])
+def test_config0_32k(mode, ncrit, group_cell):
     cfg = W.CONFIGS["plummer_32k"]
     pm = W.plummer(cfg["n"])
-    ref = O.full_step(pm, cfg["theta"], cfg["eps"], ncrit=ncrit, group_mode=mode)
-    b, out = run_gpu(pm, cfg["theta"], cfg["eps"], ncrit=ncrit, group_mode=mode)
+    ref = O.full_step(pm, cfg["theta"], cfg["eps"], ncrit=ncrit, group_mode=mode, group_cell=max(group_cell, ncrit))
+    b, out = run_gpu(pm, cfg["theta"], cfg["eps"], ncrit=ncrit, group_mode=mode, group_cell=group_cell)
     check_structure(b, ref)
     check_groups(b, ref)
     r = check_walk(b, out, ref)
@@ -193,7 +194,7 @@ def test_eps_zero():
 
 
 @pytest.mark.parametrize("pattern,frac", [("scattered", 16), ("clustered", 16), ("scattered", 256)])
-@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1, 2])
 def test_active_mask(pattern, frac, mode):
     n = 1 << 15
     pm = W.plummer(n)

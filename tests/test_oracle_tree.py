@@ -134,6 +134,43 @@ def test_groups_partition_and_boxes(step, mode, ncrit):
             assert (g.bmax[k] == spm[mem, :3].max(axis=0)).all()
 
 
+@pytest.mark.parametrize("ncrit,group_cell", [(32, 512), (64, 1024), (16, 16), (32, 1 << 30)])
+def test_groups_cell_chunk_mode(step, ncrit, group_cell):
+    """mode 2 (R13): chunks of ncrit inside the container cells (count <= group_cell, parent count > group_cell)."""
+    spm, t = step.sorted_pos_mass, step.tree
+    n = spm.shape[0]
+    # containers from the definition, by brute force over all cells
+    cont = sorted((int(t.first[i]), int(t.count[i])) for i in range(t.n_cells)
+                  if (t.count[i] <= group_cell or t.n_child[i] == 0)
+                  and (t.parent[i] == 0xFFFFFFFF or t.count[t.parent[i]] > group_cell))
+    cont = sorted(set(cont))
+    assert cont[0][0] == 0 and sum(c for _, c in cont) == n          # containers tile [0, n)
+    for act in (None, (W.uniform(5, np.arange(n, dtype=np.uint64), 0) < 0.07).astype(np.uint8)):
+        g = O.groups(2, ncrit, spm, t, act, group_cell)
+        flag = np.ones(n, bool) if act is None else act.astype(bool)
+        rank = np.concatenate([[0], np.cumsum(flag)])
+        want_first, want_count = [], []
+        for f, c in cont:
+            r0, a = rank[f], rank[f + c] - rank[f]
+            for o in range(0, a, ncrit):
+                want_first.append(r0 + o)
+                want_count.append(min(ncrit, a - o))
+        assert g.n_groups == len(want_first)
+        assert (g.first == np.array(want_first)).all() and (g.count == np.array(want_count)).all()
+        assert (g.active_list == np.nonzero(flag)[0]).all()
+        for k in range(0, g.n_groups, max(1, g.n_groups // 50)):
+            mem = g.active_list[g.first[k]:g.first[k] + g.count[k]]
+            assert (g.bmin[k] == spm[mem, :3].min(axis=0)).all()
+            assert (g.bmax[k] == spm[mem, :3].max(axis=0)).all()
+    # limits: group_cell = ncrit reproduces mode 0, group_cell >= n reproduces mode 1
+    if group_cell == ncrit:
+        g0, g2 = O.groups(0, ncrit, spm, t), O.groups(2, ncrit, spm, t, None, group_cell)
+        assert (g0.first == g2.first).all() and (g0.count == g2.count).all()
+    if group_cell >= n:
+        g1, g2 = O.groups(1, ncrit, spm, t), O.groups(2, ncrit, spm, t, None, group_cell)
+        assert (g1.first == g2.first).all() and (g1.count == g2.count).all()
+
+
 def _brute(spm, b, e):
     x = spm[b:e, :3].astype(np.float64)
     m = spm[b:e, 3].astype(np.float64)
