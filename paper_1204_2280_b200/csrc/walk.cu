@@ -40,6 +40,7 @@ struct __align__(16) WarpSmem {
     uint32_t pc_ids[64];           // ring of accepted cell ids
     uint32_t leaf_first[32];
     uint32_t leaf_pref[36];
+    float2 sink_xyz[3][32];        // per lane: negated (x0, x1), (y0, y1), (z0, z1) of its two sinks, see walk_chunk
 };
 
 size_t walk_smem_bytes(uint32_t) { return sizeof(WarpSmem) * kWalkWarps; }
@@ -50,14 +51,87 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
     return y;
 }
 
+// Packed fp32x2 arithmetic (sm_100: FFMA2 / FMUL2 / FADD2).  One instruction does the same IEEE operation on the
+// two halves of a 64-bit register pair, so a lane that holds two sinks spends ONE issue slot per operation for
+// both of them.  Measured on B200 (profiles/r1b_fp32_peak_microbench.txt): FFMA2 runs at half the instruction rate
+// of FFMA -- the same 74 TFLOP/s -- which turns the interaction loops from issue-bound into FP32-pipe-bound.
+typedef unsigned long long f32x2;  // two fp32 values in one 64-bit register pair: .x = low half, .y = high half
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float lo2(f32x2 v) {
+    float a, b;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+    return a;
+}
+__device__ __forceinline__ float hi2(f32x2 v) {
+    float a, b;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+    return b;
+}
+__device__ __forceinline__ f32x2 bc(float v) { return pack2(v, v); }
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 rsqrt2(f32x2 v) { return pack2(rsqrt_fast(lo2(v)), rsqrt_fast(hi2(v))); }
+
 template <int NS>
 struct Sinks {
+    f32x2 nx2, ny2, nz2;     // NS = 2: (-x0, -x1), (-y0, -y1), (-z0, -z1), kept packed for the whole walk
     float x[NS], y[NS], z[NS];
     double ax[NS], ay[NS], az[NS], ph[NS];  // ph accumulates +sum m/r (negated on output)
 };
 
+// NS = 2: the two sinks of a lane ride in the two halves of packed registers; operation for operation (and
+// rounding for rounding) the same arithmetic as the scalar loop below.
+template <bool kZeroEps>
+__device__ __forceinline__ void eval_pp_packed(WarpSmem& S, uint32_t r0, int nb, float eps2, Sinks<2>& s) {
+    const f32x2 nsx = s.nx2, nsy = s.ny2, nsz = s.nz2;
+    const f32x2 e2 = bc(eps2);
+    f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
+#pragma unroll 4
+    for (int j = 0; j < nb; ++j) {
+        const float4 q = S.pp[(r0 + j) & 63];
+        const f32x2 dx = fadd2(bc(q.x), nsx), dy = fadd2(bc(q.y), nsy), dz = fadd2(bc(q.z), nsz);
+        f32x2 rinv;
+        if (kZeroEps) {
+            const f32x2 r2 = ffma2(dx, dx, ffma2(dy, dy, fmul2(dz, dz)));
+            rinv = pack2((lo2(r2) > 0.0f) ? rsqrt_fast(lo2(r2)) : 0.0f, (hi2(r2) > 0.0f) ? rsqrt_fast(hi2(r2)) : 0.0f);
+        } else {
+            rinv = rsqrt2(ffma2(dx, dx, ffma2(dy, dy, ffma2(dz, dz, e2))));
+        }
+        const f32x2 mr = fmul2(bc(q.w), rinv);
+        const f32x2 rinv2 = fmul2(rinv, rinv);
+        const f32x2 mr3 = fmul2(mr, rinv2);
+        ph = fadd2(ph, mr);
+        ax = ffma2(mr3, dx, ax);
+        ay = ffma2(mr3, dy, ay);
+        az = ffma2(mr3, dz, az);
+    }
+    s.ax[0] += (double)lo2(ax); s.ay[0] += (double)lo2(ay); s.az[0] += (double)lo2(az); s.ph[0] += (double)lo2(ph);
+    s.ax[1] += (double)hi2(ax); s.ay[1] += (double)hi2(ay); s.az[1] += (double)hi2(az); s.ph[1] += (double)hi2(ph);
+    __syncwarp();
+}
+
 template <int NS, bool kZeroEps>
 __device__ __forceinline__ void eval_pp(WarpSmem& S, uint32_t r0, int nb, float eps2, Sinks<NS>& s) {
+    if constexpr (NS == 2) {
+        eval_pp_packed<kZeroEps>(S, r0, nb, eps2, s);
+    } else {
     float ax[NS], ay[NS], az[NS], ph[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) ax[k] = ay[k] = az[k] = ph[k] = 0.0f;
@@ -88,6 +162,7 @@ __device__ __forceinline__ void eval_pp(WarpSmem& S, uint32_t r0, int nb, float 
         s.ax[k] += (double)ax[k]; s.ay[k] += (double)ay[k]; s.az[k] += (double)az[k]; s.ph[k] += (double)ph[k];
     }
     __syncwarp();
+    }
 }
 
 template <int NS>
@@ -101,6 +176,37 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
         S.pc[lane][2] = __ldg(q + 1);
     }
     __syncwarp();
+    if constexpr (NS == 2) {
+        const f32x2 nsx = s.nx2, nsy = s.ny2, nsz = s.nz2;
+        const f32x2 e2 = bc(a.eps2);
+        f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
+#pragma unroll 2
+        for (int j = 0; j < nb; ++j) {
+            const float4 c0 = S.pc[j][0], c1 = S.pc[j][1], c2 = S.pc[j][2];
+            const f32x2 dx = fadd2(bc(c0.x), nsx), dy = fadd2(bc(c0.y), nsy), dz = fadd2(bc(c0.z), nsz);
+            const f32x2 rinv = rsqrt2(ffma2(dx, dx, ffma2(dy, dy, ffma2(dz, dz, e2))));
+            const f32x2 rinv2 = fmul2(rinv, rinv);
+            const f32x2 qrx = ffma2(bc(c1.x), dx, ffma2(bc(c1.w), dy, fmul2(bc(c2.x), dz)));
+            const f32x2 qry = ffma2(bc(c1.w), dx, ffma2(bc(c1.y), dy, fmul2(bc(c2.y), dz)));
+            const f32x2 qrz = ffma2(bc(c2.x), dx, ffma2(bc(c2.y), dy, fmul2(bc(c1.z), dz)));
+            const f32x2 qq = ffma2(dx, qrx, ffma2(dy, qry, fmul2(dz, qrz)));
+            const f32x2 rinv3 = fmul2(rinv, rinv2);
+            const f32x2 rinv5 = fmul2(rinv3, rinv2);
+            const f32x2 q5 = fmul2(qq, rinv5);
+            ph = ffma2(bc(c0.w), rinv, ph);
+            ph = ffma2(bc(c2.z), rinv3, ph);
+            ph = ffma2(bc(1.5f), q5, ph);
+            f32x2 f = ffma2(bc(7.5f), fmul2(q5, rinv2), fmul2(bc(c2.w), rinv5));
+            f = ffma2(bc(c0.w), rinv3, f);
+            const f32x2 g = fmul2(bc(-3.0f), rinv5);
+            ax = ffma2(dx, f, ax); ax = ffma2(g, qrx, ax);
+            ay = ffma2(dy, f, ay); ay = ffma2(g, qry, ay);
+            az = ffma2(dz, f, az); az = ffma2(g, qrz, az);
+        }
+        s.ax[0] += (double)lo2(ax); s.ay[0] += (double)lo2(ay); s.az[0] += (double)lo2(az); s.ph[0] += (double)lo2(ph);
+        s.ax[1] += (double)hi2(ax); s.ay[1] += (double)hi2(ay); s.az[1] += (double)hi2(az); s.ph[1] += (double)hi2(ph);
+        __syncwarp();
+    } else {
     float ax[NS], ay[NS], az[NS], ph[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) ax[k] = ay[k] = az[k] = ph[k] = 0.0f;
@@ -138,6 +244,7 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
         s.ax[k] += (double)ax[k]; s.ay[k] += (double)ay[k]; s.az[k] += (double)az[k]; s.ph[k] += (double)ph[k];
     }
     __syncwarp();
+    }
 }
 
 // Walk one chunk (<= 32 NS sinks) of group g.  Returns false on stack overflow.
@@ -156,6 +263,20 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
         s.x[k] = p.x; s.y[k] = p.y; s.z[k] = p.z;
         smass[k] = p.w;
         s.ax[k] = s.ay[k] = s.az[k] = s.ph[k] = 0.0;
+    }
+    if constexpr (NS == 2) {
+        // The packed loops want (-x0, -x1) etc. in ALIGNED register pairs.  Left as halves of the two float4 loads
+        // above, ptxas re-pairs them with two MOVs per coordinate in every loop iteration (ALU-pipe slots that
+        // FFMA2 cannot overlap, profiles/r1c); a round trip through shared memory as 64-bit words makes each pair
+        // the destination of one LDS.64.
+        S.sink_xyz[0][lane] = make_float2(-s.x[0], -s.x[1]);
+        S.sink_xyz[1][lane] = make_float2(-s.y[0], -s.y[1]);
+        S.sink_xyz[2][lane] = make_float2(-s.z[0], -s.z[1]);
+        __syncwarp();
+        const uint32_t sa = (uint32_t)__cvta_generic_to_shared(&S.sink_xyz[0][lane]);
+        asm volatile("ld.shared.b64 %0, [%1];" : "=l"(s.nx2) : "r"(sa));
+        asm volatile("ld.shared.b64 %0, [%1];" : "=l"(s.ny2) : "r"(sa + 256u));
+        asm volatile("ld.shared.b64 %0, [%1];" : "=l"(s.nz2) : "r"(sa + 512u));
     }
     uint32_t pc_r = 0, pc_w = 0, pp_r = 0, pp_w = 0;
     uint32_t npc = 0, npp = 0;
@@ -288,7 +409,7 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
 }
 
 template <bool kZeroEps>
-__global__ void __launch_bounds__(kWalkWarps * 32) k_walk(WalkArgs a) {
+__global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[w];
