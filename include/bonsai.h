@@ -145,8 +145,10 @@ typedef struct {
                                       f32 COM x, y, z, mass, delta = |COM - geometric centre|, l = cell side,
                                       then u32 link (leaf: first particle; else first child) and u32 info
                                       (leaf: 0x80000000 | count; else n_child)                                */
-    const float* quad;             /* device, 8 floats per cell: xx, yy, zz, xy, xz, yz (raw second moments
-                                      about the COM, R8), then -tr/2 and -3 tr/2 as the walk uses them       */
+    const float* quad;             /* device, 6 floats per cell: xx, yy, zz, xy, xz, yz (raw second moments
+                                      about the COM, R8)                                                     */
+    const float* walk_quad;        /* device, 8 floats per cell, the walk's second record: P = tr I - 3 Q as
+                                      Pxx, Pyy, Pzz, Pxy, Pxz, Pyz, then tr = Qxx + Qyy + Qzz and a pad      */
 } bonsai_cells_view;
 int bonsai_get_cells(bonsai_ctx* ctx, bonsai_cells_view* out);
 

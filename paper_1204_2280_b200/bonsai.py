@@ -39,7 +39,7 @@ class Params(C.Structure):
 class CellsView(C.Structure):
     _fields_ = [("cap_cells", C.c_uint32)] + [(k, C.c_void_p) for k in (
         "n_cells", "level_offsets", "level", "first", "count", "first_child", "n_child", "parent",
-        "mac", "quad")]
+        "mac", "quad", "walk_quad")]
 
 
 class GroupsView(C.Structure):
@@ -127,6 +127,7 @@ class Cells:
     quad: "object" = None    # float32[n_cells, 6]
     delta: "object" = None
     lside: "object" = None
+    walk_quad: "object" = None  # float32[n_cells, 8]: P = tr I - 3 Q (6), tr, pad
 
 
 @dataclass
@@ -314,11 +315,12 @@ class Bonsai:
                     u(v.first_child), u(v.n_child), u(v.parent))
         if with_multipoles:
             mac = self._host(v.mac, 8 * nc, torch.float32).reshape(nc, 8)
-            quad = self._host(v.quad, 8 * nc, torch.float32).reshape(nc, 8)
+            quad = self._host(v.quad, 6 * nc, torch.float32).reshape(nc, 6)
             out.com_m = mac[:, :4].copy()
             out.delta = mac[:, 4].copy()
             out.lside = mac[:, 5].copy()
-            out.quad = quad[:, :6].copy()
+            out.quad = quad
+            out.walk_quad = self._host(v.walk_quad, 8 * nc, torch.float32).reshape(nc, 8)
         return out
 
     def groups(self) -> Groups:

@@ -82,6 +82,7 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     t.c_parent = cv.take<uint32_t>(cap);
     t.c_mac = cv.take<CellMac>(cap);
     t.c_quad = cv.take<CellQuad>(cap);
+    t.c_qraw = cv.take<float>(cap * 6);
     t.c_mom = cv.take<double>(cap * 10);
     t.c_arrived = cv.take<uint32_t>(cap);
     t.rank = cv.take<uint32_t>((size_t)n + 1);
@@ -310,7 +311,8 @@ int bonsai_get_cells(bonsai_ctx* h, bonsai_cells_view* out) {
     out->n_child = b.c_n_child;
     out->parent = b.c_parent;
     out->mac = reinterpret_cast<const float*>(b.c_mac);
-    out->quad = reinterpret_cast<const float*>(b.c_quad);
+    out->quad = b.c_qraw;
+    out->walk_quad = reinterpret_cast<const float*>(b.c_quad);
     return BONSAI_OK;
 }
 

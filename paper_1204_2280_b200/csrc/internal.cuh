@@ -61,9 +61,13 @@ struct __align__(16) CellMac {
     uint32_t info;             // internal: n_child (1..8);  leaf: kLeafBit | count
 };
 struct __align__(16) CellQuad {
-    float xx, yy, zz, xy, xz, yz;  // raw second moments about the COM
-    float mtr_half;                // -1/2 (xx + yy + zz)
-    float mtr_3half;               // -3/2 (xx + yy + zz)
+    // P = tr I - 3 Q  (minus the trace-free quadrupole; Q = raw second moments about the COM, tr = Qxx + Qyy + Qzz),
+    // formed in fp64 and rounded once.  With r^2 = |dr|^2 + eps^2 in every power (R10) the raw-moment formulas are
+    //   phi = -M/r + (dr.P.dr + tr eps^2) / (2 r^5),   a = dr (M/r^3 - 5 (dr.P.dr + tr eps^2) / (2 r^7)) + P.dr / r^5
+    // exactly, which is 33 FP32 operations per particle-cell interaction instead of 36 (walk.cu).
+    float pxx, pyy, pzz, pxy, pxz, pyz;
+    float tr;
+    float pad;
 };
 
 struct Buffers {
@@ -84,6 +88,7 @@ struct Buffers {
     // multipoles
     CellMac* c_mac;            // [cap]
     CellQuad* c_quad;          // [cap]
+    float* c_qraw;             // [cap][6] raw second moments xx, yy, zz, xy, xz, yz as fp32 (introspection, R8)
     double* c_mom;             // [cap][10] fp64: M, COMx, COMy, COMz, Qxx, Qyy, Qzz, Qxy, Qxz, Qyz
     uint32_t* c_arrived;       // [cap] children that have finished
     // groups

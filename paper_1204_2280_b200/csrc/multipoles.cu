@@ -29,7 +29,7 @@ struct Mom {
 __device__ __forceinline__ void store_cell(const Mom& q, uint32_t c, int L, uint32_t khi, uint32_t kmid, uint32_t klo,
                                            const Control* __restrict__ ctl, uint32_t link_first, uint32_t link_info,
                                            double* __restrict__ c_mom, CellMac* __restrict__ c_mac,
-                                           CellQuad* __restrict__ c_quad) {
+                                           CellQuad* __restrict__ c_quad, float* __restrict__ c_qraw) {
     // geometric centre: integer cell coordinate = top L bits of the quantised coordinate of any member (R8)
     const double l = ldexp(ctl->side, -L);
     double g[3];
@@ -58,12 +58,15 @@ __device__ __forceinline__ void store_cell(const Mom& q, uint32_t c, int L, uint
     cm.first = link_first;
     cm.info = link_info;
     c_mac[c] = cm;
+    float* qr = c_qraw + (size_t)c * 6;
+    qr[0] = (float)o.xx; qr[1] = (float)o.yy; qr[2] = (float)o.zz;
+    qr[3] = (float)o.xy; qr[4] = (float)o.xz; qr[5] = (float)o.yz;
+    const double tr = o.xx + o.yy + o.zz;
     CellQuad cq;
-    cq.xx = (float)o.xx; cq.yy = (float)o.yy; cq.zz = (float)o.zz;
-    cq.xy = (float)o.xy; cq.xz = (float)o.xz; cq.yz = (float)o.yz;
-    const float tr = (cq.xx + cq.yy) + cq.zz;
-    cq.mtr_half = -0.5f * tr;
-    cq.mtr_3half = -1.5f * tr;
+    cq.pxx = (float)(tr - 3.0 * o.xx); cq.pyy = (float)(tr - 3.0 * o.yy); cq.pzz = (float)(tr - 3.0 * o.zz);
+    cq.pxy = (float)(-3.0 * o.xy); cq.pxz = (float)(-3.0 * o.xz); cq.pyz = (float)(-3.0 * o.yz);
+    cq.tr = (float)tr;
+    cq.pad = 0.0f;
     c_quad[c] = cq;
 }
 
@@ -76,7 +79,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
                                                     const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
                                                     const uint32_t* __restrict__ klo, double* __restrict__ c_mom,
                                                     CellMac* __restrict__ c_mac, CellQuad* __restrict__ c_quad,
-                                                    uint32_t* __restrict__ c_arrived) {
+                                                    float* __restrict__ c_qraw, uint32_t* __restrict__ c_arrived) {
     uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= min(ctl->n_cells, cap_cells)) return;
     if (t.n_child[c] != 0) return;  // internal cells are produced by their last child
@@ -111,7 +114,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
             }
         }
         store_cell(q, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f, kLeafBit | cnt, c_mom,
-                   c_mac, c_quad);
+                   c_mac, c_quad, c_qraw);
     }
     for (;;) {
         const uint32_t p = t.parent[c];
@@ -152,7 +155,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         }
         const uint32_t f = t.first[p];
         store_cell(q, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc, c_mom, c_mac,
-                   c_quad);
+                   c_quad, c_qraw);
         c = p;
     }
 }
@@ -163,7 +166,7 @@ cudaError_t stage_multipoles(Ctx* c) {
     TreeView t{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
     k_multipoles<<<div_up(c->cap_cells, 128), 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0],
                                                                    b.key[s][1], b.key[s][2], b.c_mom, b.c_mac, b.c_quad,
-                                                                   b.c_arrived);
+                                                                   b.c_qraw, b.c_arrived);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -35,7 +35,7 @@ struct WalkArgs {
 
 struct __align__(16) WarpSmem {
     float4 pp[64];                 // ring of p-p sources
-    float4 pc[32][3];              // staged p-c sources: (cx,cy,cz,m) (xx,yy,zz,xy) (xz,yz,-tr/2,-3tr/2)
+    float4 pc[32][3];              // staged p-c sources: (cx,cy,cz,m) (Pxx,Pyy,Pzz,Pxy) (Pxz,Pyz,tr eps^2,-)
     uint32_t stack[kWalkStack];    // runs of sibling cells: (first << 3) | (n - 1)
     uint32_t pc_ids[64];           // ring of accepted cell ids
     uint32_t leaf_first[32];
@@ -103,9 +103,10 @@ __device__ __forceinline__ void eval_pp_packed(WarpSmem& S, uint32_t r0, int nb,
     const f32x2 nsx = s.nx2, nsy = s.ny2, nsz = s.nz2;
     const f32x2 e2 = bc(eps2);
     f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
+    const float4* src = &S.pp[r0 & 63u];  // batches start at ring slot 0 or 32 and hold <= 32 sources: no wrap
 #pragma unroll 4
     for (int j = 0; j < nb; ++j) {
-        const float4 q = S.pp[(r0 + j) & 63];
+        const float4 q = src[j];
         const f32x2 dx = fadd2(bc(q.x), nsx), dy = fadd2(bc(q.y), nsy), dz = fadd2(bc(q.z), nsz);
         f32x2 rinv;
         if (kZeroEps) {
@@ -135,9 +136,10 @@ __device__ __forceinline__ void eval_pp(WarpSmem& S, uint32_t r0, int nb, float 
     float ax[NS], ay[NS], az[NS], ph[NS];
 #pragma unroll
     for (int k = 0; k < NS; ++k) ax[k] = ay[k] = az[k] = ph[k] = 0.0f;
+    const float4* src = &S.pp[r0 & 63u];
 #pragma unroll 4
     for (int j = 0; j < nb; ++j) {
-        const float4 q = S.pp[(r0 + j) & 63];
+        const float4 q = src[j];
 #pragma unroll
         for (int k = 0; k < NS; ++k) {
             const float dx = q.x - s.x[k], dy = q.y - s.y[k], dz = q.z - s.z[k];
@@ -173,7 +175,9 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
         const float4* q = reinterpret_cast<const float4*>(a.quad + c);
         S.pc[lane][0] = __ldg(m);
         S.pc[lane][1] = __ldg(q);
-        S.pc[lane][2] = __ldg(q + 1);
+        float4 q1 = __ldg(q + 1);
+        q1.z = q1.z * a.eps2;  // tr eps^2: the softening term of the quadrupole (see CellQuad), once per cell
+        S.pc[lane][2] = q1;
     }
     __syncwarp();
     if constexpr (NS == 2) {
@@ -186,22 +190,22 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
             const f32x2 dx = fadd2(bc(c0.x), nsx), dy = fadd2(bc(c0.y), nsy), dz = fadd2(bc(c0.z), nsz);
             const f32x2 rinv = rsqrt2(ffma2(dx, dx, ffma2(dy, dy, ffma2(dz, dz, e2))));
             const f32x2 rinv2 = fmul2(rinv, rinv);
-            const f32x2 qrx = ffma2(bc(c1.x), dx, ffma2(bc(c1.w), dy, fmul2(bc(c2.x), dz)));
-            const f32x2 qry = ffma2(bc(c1.w), dx, ffma2(bc(c1.y), dy, fmul2(bc(c2.y), dz)));
-            const f32x2 qrz = ffma2(bc(c2.x), dx, ffma2(bc(c2.y), dy, fmul2(bc(c1.z), dz)));
-            const f32x2 qq = ffma2(dx, qrx, ffma2(dy, qry, fmul2(dz, qrz)));
+            // c1 = (Pxx, Pyy, Pzz, Pxy), c2 = (Pxz, Pyz, tr eps^2, -)
+            const f32x2 prx = ffma2(bc(c1.x), dx, ffma2(bc(c1.w), dy, fmul2(bc(c2.x), dz)));
+            const f32x2 pry = ffma2(bc(c1.w), dx, ffma2(bc(c1.y), dy, fmul2(bc(c2.y), dz)));
+            const f32x2 prz = ffma2(bc(c2.x), dx, ffma2(bc(c2.y), dy, fmul2(bc(c1.z), dz)));
+            const f32x2 sq = ffma2(dx, prx, ffma2(dy, pry, ffma2(dz, prz, bc(c2.z))));  // dr.P.dr + tr eps^2
             const f32x2 rinv3 = fmul2(rinv, rinv2);
             const f32x2 rinv5 = fmul2(rinv3, rinv2);
-            const f32x2 q5 = fmul2(qq, rinv5);
+            const f32x2 q5 = fmul2(sq, rinv5);
+            // ph accumulates -phi = M/r - (dr.P.dr + tr eps^2) / (2 r^5)
             ph = ffma2(bc(c0.w), rinv, ph);
-            ph = ffma2(bc(c2.z), rinv3, ph);
-            ph = ffma2(bc(1.5f), q5, ph);
-            f32x2 f = ffma2(bc(7.5f), fmul2(q5, rinv2), fmul2(bc(c2.w), rinv5));
-            f = ffma2(bc(c0.w), rinv3, f);
-            const f32x2 g = fmul2(bc(-3.0f), rinv5);
-            ax = ffma2(dx, f, ax); ax = ffma2(g, qrx, ax);
-            ay = ffma2(dy, f, ay); ay = ffma2(g, qry, ay);
-            az = ffma2(dz, f, az); az = ffma2(g, qrz, az);
+            ph = ffma2(bc(-0.5f), q5, ph);
+            // a = dr (M/r^3 - 5/2 q5/r^2) + P.dr / r^5
+            const f32x2 f = ffma2(bc(-2.5f), fmul2(q5, rinv2), fmul2(bc(c0.w), rinv3));
+            ax = ffma2(dx, f, ax); ax = ffma2(rinv5, prx, ax);
+            ay = ffma2(dy, f, ay); ay = ffma2(rinv5, pry, ay);
+            az = ffma2(dz, f, az); az = ffma2(rinv5, prz, az);
         }
         s.ax[0] += (double)lo2(ax); s.ay[0] += (double)lo2(ay); s.az[0] += (double)lo2(az); s.ph[0] += (double)lo2(ph);
         s.ax[1] += (double)hi2(ax); s.ay[1] += (double)hi2(ay); s.az[1] += (double)hi2(az); s.ph[1] += (double)hi2(ph);
@@ -219,24 +223,19 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
             const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.eps2)));
             const float rinv = rsqrt_fast(r2);
             const float rinv2 = rinv * rinv;
-            const float qrx = fmaf(c1.x, dx, fmaf(c1.w, dy, c2.x * dz));
-            const float qry = fmaf(c1.w, dx, fmaf(c1.y, dy, c2.y * dz));
-            const float qrz = fmaf(c2.x, dx, fmaf(c2.y, dy, c1.z * dz));
-            const float qq = fmaf(dx, qrx, fmaf(dy, qry, dz * qrz));
+            const float prx = fmaf(c1.x, dx, fmaf(c1.w, dy, c2.x * dz));
+            const float pry = fmaf(c1.w, dx, fmaf(c1.y, dy, c2.y * dz));
+            const float prz = fmaf(c2.x, dx, fmaf(c2.y, dy, c1.z * dz));
+            const float sq = fmaf(dx, prx, fmaf(dy, pry, fmaf(dz, prz, c2.z)));
             const float rinv3 = rinv * rinv2;
             const float rinv5 = rinv3 * rinv2;
-            const float q5 = qq * rinv5;
-            // phi = -(M/r - tr/(2 r^3) + 3 q/(2 r^5))
+            const float q5 = sq * rinv5;
             ph[k] = fmaf(c0.w, rinv, ph[k]);
-            ph[k] = fmaf(c2.z, rinv3, ph[k]);
-            ph[k] = fmaf(1.5f, q5, ph[k]);
-            // a = dr (M/r^3 - 3 tr/(2 r^5) + 15 q/(2 r^7)) - 3 Q dr / r^5
-            float f = fmaf(7.5f, q5 * rinv2, c2.w * rinv5);
-            f = fmaf(c0.w, rinv3, f);
-            const float g = -3.0f * rinv5;
-            ax[k] = fmaf(dx, f, ax[k]); ax[k] = fmaf(g, qrx, ax[k]);
-            ay[k] = fmaf(dy, f, ay[k]); ay[k] = fmaf(g, qry, ay[k]);
-            az[k] = fmaf(dz, f, az[k]); az[k] = fmaf(g, qrz, az[k]);
+            ph[k] = fmaf(-0.5f, q5, ph[k]);
+            const float f = fmaf(-2.5f, q5 * rinv2, c0.w * rinv3);
+            ax[k] = fmaf(dx, f, ax[k]); ax[k] = fmaf(rinv5, prx, ax[k]);
+            ay[k] = fmaf(dy, f, ay[k]); ay[k] = fmaf(rinv5, pry, ay[k]);
+            az[k] = fmaf(dz, f, az[k]); az[k] = fmaf(rinv5, prz, az[k]);
         }
     }
 #pragma unroll

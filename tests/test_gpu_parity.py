@@ -276,3 +276,36 @@ def test_errors():
     with pytest.raises(BonsaiError) as e:
         b2.sync()
     assert e.value.code == -3
+
+
+def test_full_size_4m_sampled():
+    """BASELINE.json configs[3] (the workload bench.py times: N = 2^22, theta 0.75, eps 0.00125, default groups).
+
+    Every structural stage is compared in full (bit-exact; multipoles <= 1 ulp); the walk is compared on the sinks of
+    an evenly spaced sample of groups, which the oracle walks one by one."""
+    cfg = W.CONFIGS["plummer_4m"]
+    n, theta, eps = cfg["n"], cfg["theta"], cfg["eps"]
+    pm = W.plummer(n)
+    ref = O.build(pm)
+    b, out = run_gpu(pm, theta, eps)
+    check_structure(b, ref)
+    check_groups(b, ref)
+    g = ref.groups
+    sel = np.arange(0, g.n_groups, max(1, g.n_groups // 256), dtype=np.uint32)
+    w = O.walk(theta, eps, ref.sorted_pos_mass, ref.tree, g, sel)
+    n_pp, n_pc = b.counts()
+    perm = ref.perm
+    sinks = np.concatenate([g.active_list[g.first[k]: g.first[k] + g.count[k]] for k in sel])   # sorted indices
+    border = np.concatenate([np.full(g.count[k], bool(w.g_borderline[i])) for i, k in enumerate(sel)])
+    load = perm[sinks]
+    same = (n_pp[load] == w.n_pp[sinks]) & (n_pc[load] == w.n_pc[sinks])
+    assert same.mean() >= 0.999 or not (~same & ~border).any(), same.mean()
+    assert not (~same & ~border).any()
+    ea, ep = _rel_err(out[load[same], :3].astype(np.float64), out[load[same], 3].astype(np.float64),
+                      w.acc[sinks[same]], w.pot[sinks[same]])
+    assert ea.max() <= ACC_MAX and ep.max() <= ACC_MAX, (ea.max(), ep.max())
+    assert np.median(ea) <= ACC_MEDIAN and np.median(ep) <= ACC_MEDIAN, (np.median(ea), np.median(ep))
+    # totals agree with the per-particle counters
+    spp, spc = b.interaction_totals()
+    assert spp == int(n_pp.astype(np.int64).sum()) and spc == int(n_pc.astype(np.int64).sum())
+    print("4m sampled", len(sinks), float(same.mean()), float(ea.max()), float(np.median(ea)), float(ep.max()))
