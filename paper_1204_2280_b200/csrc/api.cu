@@ -64,10 +64,11 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     t.ctl = cv.take<Control>(1);
     for (int k = 0; k < 2; ++k) {
         for (int w = 0; w < 3; ++w) t.key[k][w] = cv.take<uint32_t>(n);
+        t.pair_key[k] = cv.take<uint32_t>(n);
         t.idx[k] = cv.take<uint32_t>(n);
     }
     t.ghist = cv.take<uint32_t>((size_t)kSortPasses * kRadix);
-    t.tile_count = cv.take<uint32_t>((size_t)kRadix * n_tiles);
+    t.look = cv.take<unsigned long long>((size_t)kRadix * n_tiles);
     t.bbox_partial = cv.take<float>(6 * 148 * 16);
     t.sorted_pos = cv.take<float4>(n);
     t.lcp = cv.take<int8_t>((size_t)n + 1);
@@ -152,7 +153,9 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.stream = static_cast<cudaStream_t>(cuda_stream);
     carve(static_cast<unsigned char*>(workspace_dev), n_max, p, &c.b);
     c.pos_mass = nullptr;
-    c.sorted_buf = 0;
+    c.sorted_buf = 1;
+    c.perm = c.b.idx[0];
+    c.sort_epoch = 0;
     c.state = 0;
     c.groups_all_active = false;
     c.timing = false;
@@ -167,8 +170,11 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
         delete h;
         return BONSAI_ECUDA;
     }
-    // control block and the self-cleaning arrival counters start at zero
+    // control block, the self-cleaning arrival counters and the sort's look-back table (epoch 0 = never written)
+    // start at zero
     if (cudaMemsetAsync(c.b.ctl, 0, sizeof(Control), c.stream) != cudaSuccess ||
+        cudaMemsetAsync(c.b.look, 0, sizeof(unsigned long long) * (size_t)kRadix * div_up(n_max, kSortTile), c.stream) !=
+            cudaSuccess ||
         cudaMemsetAsync(c.b.c_arrived, 0, sizeof(uint32_t) * (size_t)c.cap_cells, c.stream) != cudaSuccess) {
         delete h;
         return BONSAI_ECUDA;
@@ -286,7 +292,7 @@ int bonsai_get_keys(bonsai_ctx* h, const uint32_t** hi_dev, const uint32_t** mid
 int bonsai_get_perm(bonsai_ctx* h, const uint32_t** perm_dev) {
     if (!h || !perm_dev) return BONSAI_EINVAL;
     if (h->c.state < 2) return BONSAI_ESTATE;
-    *perm_dev = h->c.b.idx[h->c.sorted_buf];
+    *perm_dev = h->c.perm;
     return BONSAI_OK;
 }
 

@@ -141,7 +141,7 @@ cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order) {
         k_groups_identity<<<div_up(n + 1, 256), 256, 0, c->stream>>>(n, b.rank, b.active_list, b.ctl);
         c->launches += 1;
     } else {
-        k_groups_flags<<<div_up(n, 256), 256, 0, c->stream>>>(mask_load_order, b.idx[c->sorted_buf], n, b.rank);
+        k_groups_flags<<<div_up(n, 256), 256, 0, c->stream>>>(mask_load_order, c->perm, n, b.rank);
         c->launches += 1;
         if ((e = exclusive_scan_u32(c, b.rank, b.rank, n, b.scan_tmp)) != cudaSuccess) return e;
         k_groups_compact<<<div_up(n, 256), 256, 0, c->stream>>>(b.rank, n, b.active_list, b.ctl);

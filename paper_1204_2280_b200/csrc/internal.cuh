@@ -16,9 +16,10 @@ constexpr uint32_t kLeafBit = 0x80000000u;
 constexpr int kRadixBits = 10;             // one 30-bit key word = 3 digits -> 9 LSD passes for 90 bits
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kSortPasses = 9;
-constexpr int kSortThreads = 256;
-constexpr int kSortItems = 16;             // keys per thread per tile
+constexpr int kSortThreads = 512;
+constexpr int kSortItems = 16;             // pairs per thread per tile
 constexpr int kSortTile = kSortThreads * kSortItems;
+constexpr int kKeysThreads = 512;
 
 // ---- tree build geometry (tree.cu) -------------------------------------------------------------
 constexpr int kTreeThreads = 256;
@@ -45,7 +46,8 @@ struct Control {
     uint32_t bbox_ticket;
     uint32_t walk_ticket;      // dynamic group scheduler of the walk
     uint32_t level_ticket;     // last-block-done counter of k_tree_scan_levels
-    uint32_t pad0[2];
+    uint32_t sort_ticket;      // tile scheduler of k_sort_pass (reset by the tile that draws the last ticket)
+    uint32_t pad0[1];
     uint32_t level_offsets[32];  // first cell of level L; [31] = n_cells
     unsigned long long sum_pp;   // interaction totals of the last walk (sink-source pairs)
     unsigned long long sum_pc;
@@ -72,11 +74,13 @@ struct __align__(16) CellQuad {
 
 struct Buffers {
     Control* ctl;
-    // sort: ping-pong key records, structure of arrays
-    uint32_t* key[2][3];       // [buffer][word]: hi, mid, lo
+    // keys, structure of arrays: key[0] = load order (k_keys), key[1] = sorted order (k_reorder)
+    uint32_t* key[2][3];       // [order][word]: hi, mid, lo
+    // sort: ping-pong (30-bit word, index) pairs
+    uint32_t* pair_key[2];
     uint32_t* idx[2];
     uint32_t* ghist;           // [kSortPasses][kRadix] global digit histograms -> exclusive bases
-    uint32_t* tile_count;      // [kRadix][n_tiles] per-tile digit counts -> exclusive prefix over tiles
+    unsigned long long* look;  // [n_tiles][kRadix] decoupled look-back table of k_sort_pass
     float* bbox_partial;       // [blocks][6]
     float4* sorted_pos;
     // tree
@@ -113,7 +117,9 @@ struct Ctx {
     cudaStream_t stream;
     Buffers b;
     const float4* pos_mass;    // caller's particles (load order)
-    int sorted_buf;            // which ping-pong buffer holds the sorted keys
+    int sorted_buf;            // which key[] holds the sorted keys (1 once k_reorder has run)
+    uint32_t* perm;            // perm[i] = load index of the i-th sorted particle (one of b.idx[])
+    uint32_t sort_epoch;       // tag of the last k_sort_pass launch (30 bits, see sort.cu)
     int state;                 // 0 created, 1 loaded, 2 tree built, 3 multipoles done, 4 walked
     bool groups_all_active;    // the group list on the device is the all-active one
     bool timing;

@@ -85,7 +85,9 @@ __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, ui
 // a1  Morton keys (R1, R2, R4).  Per axis in fp32, round-to-nearest, no contraction:
 //   t = x - lo;  u = t * (2^30 / side);  i = trunc(u) clamped to [0, 2^30 - 1].
 // Octal digit of level L (1..30) = 4 x_bit + 2 y_bit + z_bit at bit 30 - L; words hi/mid/lo hold levels
-// 1-10 / 11-20 / 21-30.  One thread per particle; 16 B in, 4 x 4 B out, all coalesced.
+// 1-10 / 11-20 / 21-30.  Grid-stride, 16 B in, 3 x 4 B out, all coalesced.  The same pass builds the
+// digit histograms of all nine sort passes in shared memory (a histogram does not depend on the order
+// of the keys, so the sort never has to count again).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t spread10(uint32_t v) {  // 10 bits -> every third bit of 30
     v &= 0x3FFu;
@@ -103,54 +105,57 @@ __device__ __forceinline__ uint32_t quantise(float x, float lo, float scale) {
     return (uint32_t)u;  // truncation
 }
 
-__global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, uint32_t n, const Control* __restrict__ ctl,
-                                              uint32_t* __restrict__ khi, uint32_t* __restrict__ kmid,
-                                              uint32_t* __restrict__ klo, uint32_t* __restrict__ idx) {
-    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const float scale = ctl->scale;
-    float4 p = __ldg(&pos[i]);
-    uint32_t qx = quantise(p.x, ctl->lo[0], scale);
-    uint32_t qy = quantise(p.y, ctl->lo[1], scale);
-    uint32_t qz = quantise(p.z, ctl->lo[2], scale);
-    khi[i] = (spread10(qx >> 20) << 2) | (spread10(qy >> 20) << 1) | spread10(qz >> 20);
-    kmid[i] = (spread10(qx >> 10) << 2) | (spread10(qy >> 10) << 1) | spread10(qz >> 10);
-    klo[i] = (spread10(qx) << 2) | (spread10(qy) << 1) | spread10(qz);
-    idx[i] = i;
+// w[0] = lo word (levels 21-30), w[1] = mid, w[2] = hi: the order the LSD passes consume them in.
+__device__ __forceinline__ void morton_words(const float4 p, const float lox, const float loy, const float loz,
+                                             const float scale, uint32_t (&w)[3]) {
+    const uint32_t qx = quantise(p.x, lox, scale);
+    const uint32_t qy = quantise(p.y, loy, scale);
+    const uint32_t qz = quantise(p.z, loz, scale);
+    w[2] = (spread10(qx >> 20) << 2) | (spread10(qy >> 20) << 1) | spread10(qz >> 20);
+    w[1] = (spread10(qx >> 10) << 2) | (spread10(qy >> 10) << 1) | spread10(qz >> 10);
+    w[0] = (spread10(qx) << 2) | (spread10(qy) << 1) | spread10(qz);
 }
 
-// ------------------------------------------------------------------------------------------------
-// a2  Stable LSD radix sort of (90-bit key, index) records (R5): 9 passes of 10-bit digits (3 per key
-// word, lo word first).  Per pass:
-//   k_sort_count    per-tile digit histogram (shared-memory atomics), digit-major [digit][tile]
-//   k_sort_scan     one block per digit: exclusive prefix over tiles, plus the digit's global base taken
-//                   from the all-pass histogram that k_sort_ghist builds once per sort
-//   k_sort_scatter  stable in-tile ranking with __match_any_sync + per-warp digit counters, then the
-//                   record (3 key words + index) is written to its final slot
-// Records are kept as four u32 arrays so every read and the key-word of interest are coalesced.
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_sort_ghist(const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
-                                                    const uint32_t* __restrict__ klo, uint32_t n,
-                                                    uint32_t* __restrict__ ghist) {
+__global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict__ pos, uint32_t n,
+                                                       const Control* __restrict__ ctl, uint32_t* __restrict__ khi,
+                                                       uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
+                                                       uint32_t* __restrict__ ghist) {
     __shared__ uint32_t h[kSortPasses * kRadix];
-    for (int k = threadIdx.x; k < kSortPasses * kRadix; k += blockDim.x) h[k] = 0;
+    for (int k = threadIdx.x; k < kSortPasses * kRadix; k += kKeysThreads) h[k] = 0;
     __syncthreads();
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        uint32_t w[3] = {__ldg(&klo[i]), __ldg(&kmid[i]), __ldg(&khi[i])};
+    const float scale = ctl->scale, lox = ctl->lo[0], loy = ctl->lo[1], loz = ctl->lo[2];
+    const uint32_t lane = threadIdx.x & 31;
+    // warp-uniform trip count: the vote below needs the whole warp
+    for (uint32_t base = blockIdx.x * kKeysThreads + (threadIdx.x & ~31u); base < n; base += gridDim.x * kKeysThreads) {
+        const uint32_t i = base + lane;
+        const bool valid = i < n;
+        uint32_t w[3] = {0u, 0u, 0u};
+        if (valid) {
+            morton_words(__ldg(&pos[i]), lox, loy, loz, scale, w);
+            klo[i] = w[0];
+            kmid[i] = w[1];
+            khi[i] = w[2];
+        }
 #pragma unroll
         for (int p = 0; p < kSortPasses; ++p) {
-            uint32_t d = (w[p / 3] >> (kRadixBits * (p % 3))) & (kRadix - 1);
-            atomicAdd(&h[p * kRadix + d], 1u);
+            const uint32_t d = (w[p / 3] >> (kRadixBits * (p % 3))) & (kRadix - 1);
+            // a warp whose 32 keys share the digit (the leading digits of clustered or pre-sorted input)
+            // adds once instead of serialising 32 same-address atomics
+            const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, d, 0);
+            if (__all_sync(0xFFFFFFFFu, valid && d == d0)) {
+                if (lane == 0) atomicAdd(&h[p * kRadix + d], 32u);
+            } else if (valid) {
+                atomicAdd(&h[p * kRadix + d], 1u);
+            }
         }
     }
     __syncthreads();
-    for (int k = threadIdx.x; k < kSortPasses * kRadix; k += blockDim.x)
+    for (int k = threadIdx.x; k < kSortPasses * kRadix; k += kKeysThreads)
         if (h[k]) atomicAdd(&ghist[k], h[k]);
 }
 
 // exclusive scan of each pass's histogram: ghist[p][d] <- sum_{d' < d} ghist[p][d'].  One block per pass.
 __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ ghist) {
-    __shared__ uint32_t s[kRadix];
     __shared__ uint32_t wsum[kRadix / 32];
     uint32_t* h = ghist + blockIdx.x * kRadix;
     uint32_t v = h[threadIdx.x];
@@ -174,122 +179,229 @@ __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ gh
         wsum[l] = y - t;
     }
     __syncthreads();
-    (void)s;
     h[threadIdx.x] = x - v + wsum[w];
 }
 
-__global__ void __launch_bounds__(kSortThreads) k_sort_count(const uint32_t* __restrict__ word, uint32_t n, int shift,
-                                                             uint32_t n_tiles, uint32_t* __restrict__ tile_count) {
-    __shared__ uint32_t h[kRadix];
-    for (int k = threadIdx.x; k < kRadix; k += kSortThreads) h[k] = 0;
-    __syncthreads();
-    const uint32_t base = blockIdx.x * kSortTile;
-#pragma unroll
-    for (int r = 0; r < kSortItems; ++r) {
-        uint32_t i = base + r * kSortThreads + threadIdx.x;
-        if (i < n) atomicAdd(&h[(__ldg(&word[i]) >> shift) & (kRadix - 1)], 1u);
-    }
-    __syncthreads();
-    for (int k = threadIdx.x; k < kRadix; k += kSortThreads) tile_count[(size_t)k * n_tiles + blockIdx.x] = h[k];
-}
-
-// One block per digit: tile_count[d][t] <- ghist_base[d] + sum_{t' < t} tile_count[d][t'].
-__global__ void __launch_bounds__(256) k_sort_scan(uint32_t* __restrict__ tile_count, uint32_t n_tiles,
-                                                   const uint32_t* __restrict__ gbase) {
-    __shared__ uint32_t wsum[8];
-    __shared__ uint32_t carry;
-    uint32_t* row = tile_count + (size_t)blockIdx.x * n_tiles;
-    if (threadIdx.x == 0) carry = gbase[blockIdx.x];
-    __syncthreads();
-    const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (uint32_t t0 = 0; t0 < n_tiles; t0 += 256) {
-        uint32_t t = t0 + threadIdx.x;
-        uint32_t v = (t < n_tiles) ? row[t] : 0u;
-        uint32_t x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, o);
-            if (l >= o) x += y;
-        }
-        if (l == 31) wsum[w] = x;
-        __syncthreads();
-        uint32_t pre = carry;
-        for (int k = 0; k < w; ++k) pre += wsum[k];
-        if (t < n_tiles) row[t] = pre + x - v;
-        __syncthreads();
-        if (threadIdx.x == 255) carry = pre + x;
-        __syncthreads();
-    }
-}
-
-struct SortIO {
-    const uint32_t* in_key[3];
-    const uint32_t* in_idx;
-    uint32_t* out_key[3];
-    uint32_t* out_idx;
+// ------------------------------------------------------------------------------------------------
+// a2  Stable LSD radix sort of (90-bit key, index) records (R5): 9 passes of 10-bit digits, lo word
+// first.  Only (current 30-bit word, index) PAIRS move: a pass reads 8 B and writes 8 B per particle.
+// When the passes of one word are done the next word is fetched through the index (passes 3 and 6
+// gather mid[idx], hi[idx] from the load-order key arrays); the sorted 90-bit keys are re-derived from
+// the reordered positions in k_reorder (a key is a pure function of the position and the root cube).
+//
+// One kernel per pass, single sweep with decoupled look-back:
+//   * tiles of kSortTile pairs are handed out by an atomic ticket, so a tile's predecessors have
+//     always started;
+//   * stable in-tile ranking with __match_any_sync and per-warp digit counters (warp w owns a
+//     contiguous run of the tile, round r, lane l  ->  order = (warp, round, lane));
+//   * each tile publishes, per digit, first its own count (AGGREGATE) and, after summing its
+//     predecessors' entries back to the nearest INCLUSIVE one, its inclusive prefix; an entry is one
+//     64-bit word {epoch : 30, flag : 2, value : 32}, the epoch (one per pass launch) makes stale
+//     entries of earlier passes read as "not yet written", so the table is never cleared;
+//   * the digit's global base comes from the all-pass histogram k_keys built;
+//   * pairs are first permuted into tile-sorted order in shared memory (aliasing the counters), so
+//     the global stores are runs of consecutive addresses per digit.
+// ------------------------------------------------------------------------------------------------
+struct SortPass {
+    const uint32_t* key_in;    // MODE 1: pair keys of the previous pass
+    const uint32_t* idx_in;    // MODE 1, 2: indices of the previous pass
+    const uint32_t* src_word;  // MODE 0, 2: load-order key word of this phase
+    uint32_t* key_out;         // nullptr on the last pass
+    uint32_t* idx_out;
+    const uint32_t* gbase;     // [kRadix] exclusive digit bases of this pass
+    unsigned long long* look;  // [n_tiles][kRadix]
+    uint32_t* ticket;
+    uint32_t n, n_tiles, epoch;
+    int shift;
 };
 
-__global__ void __launch_bounds__(kSortThreads) k_sort_scatter(SortIO io, int word, int shift, uint32_t n,
-                                                               uint32_t n_tiles,
-                                                               const uint32_t* __restrict__ tile_offset) {
-    extern __shared__ uint32_t s_cnt[];  // [warps][kRadix]
+constexpr uint32_t kFlagAgg = 1u, kFlagIncl = 2u;
+
+__device__ __forceinline__ unsigned long long look_pack(uint32_t epoch, uint32_t flag, uint32_t value) {
+    return ((unsigned long long)((epoch << 2) | flag) << 32) | value;
+}
+__device__ __forceinline__ unsigned long long look_load(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void look_store(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// MODE 0: key = src_word[i], idx = i.   MODE 1: key = key_in[i], idx = idx_in[i].
+// MODE 2: idx = idx_in[i], key = src_word[idx].
+template <int MODE>
+__global__ void __launch_bounds__(kSortThreads, 2) k_sort_pass(const SortPass a) {
+    extern __shared__ __align__(16) uint32_t smem[];
     constexpr int kWarps = kSortThreads / 32;
-    const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (int k = threadIdx.x; k < kWarps * kRadix; k += kSortThreads) s_cnt[k] = 0;
+    constexpr int kDig = kRadix / kSortThreads;      // digits per thread in the per-digit steps
+    static_assert(kDig == 2, "the per-digit steps below handle two digits per thread");
+    uint32_t* s_cnt = smem;                          // [kWarps][kRadix]; later the staging area
+    uint32_t* s_tstart = smem + kWarps * kRadix;     // [kRadix] first tile-sorted slot of the digit
+    uint32_t* s_gdst = s_tstart + kRadix;            // [kRadix] global slot of tile-sorted slot 0 of the digit
+    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_wsum[kWarps];
+    const int tid = threadIdx.x, l = tid & 31, w = tid >> 5;
+
+    if (tid == 0) {
+        const uint32_t t = atomicAdd(a.ticket, 1u);
+        if (t == a.n_tiles - 1) *a.ticket = 0;  // every tile has drawn: ready for the next pass
+        s_tile = t;
+    }
+    {
+        uint4* z = reinterpret_cast<uint4*>(s_cnt);
+        for (int k = tid; k < kWarps * kRadix / 4; k += kSortThreads) z[k] = make_uint4(0, 0, 0, 0);
+    }
     __syncthreads();
+    const uint32_t tile = s_tile;
+    const uint32_t base_w = tile * kSortTile + w * (32 * kSortItems);
     uint32_t* cnt = s_cnt + w * kRadix;
-    // warp w owns the contiguous run [base_w, base_w + 32 * kSortItems) of the tile: round r, lane l
-    const uint32_t base_w = blockIdx.x * kSortTile + w * (32 * kSortItems);
-    const uint32_t* __restrict__ wsrc = io.in_key[word];
-    uint32_t dig[kSortItems];
+
+    uint32_t key[kSortItems];
     uint32_t rnk[kSortItems];
+    if (MODE == 2) {
+#pragma unroll
+        for (int r = 0; r < kSortItems; ++r) {
+            const uint32_t i = base_w + r * 32 + l;
+            rnk[r] = (i < a.n) ? __ldg(&a.idx_in[i]) : 0u;
+        }
+#pragma unroll
+        for (int r = 0; r < kSortItems; ++r) key[r] = __ldg(&a.src_word[rnk[r]]);
+    } else {
+        const uint32_t* __restrict__ src = (MODE == 0) ? a.src_word : a.key_in;
+#pragma unroll
+        for (int r = 0; r < kSortItems; ++r) {
+            const uint32_t i = base_w + r * 32 + l;
+            key[r] = (i < a.n) ? __ldg(&src[i]) : 0u;
+        }
+    }
     const uint32_t lt = (1u << l) - 1u;
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
-        uint32_t i = base_w + r * 32 + l;
-        bool valid = i < n;
-        uint32_t d = valid ? ((__ldg(&wsrc[i]) >> shift) & (kRadix - 1)) : (uint32_t)kRadix;  // kRadix = "no key"
-        uint32_t peers = __match_any_sync(0xFFFFFFFFu, d);
+        const bool valid = base_w + r * 32 + l < a.n;
+        const uint32_t d = valid ? ((key[r] >> a.shift) & (kRadix - 1)) : (uint32_t)kRadix;  // kRadix = "no key"
+        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, d);
         uint32_t pre = 0;
         if (valid) pre = cnt[d];
         __syncwarp();
         if (valid && (peers & lt) == 0) cnt[d] = pre + __popc(peers);
         __syncwarp();
-        dig[r] = d;
         rnk[r] = pre + __popc(peers & lt);
     }
     __syncthreads();
-    // per digit: exclusive prefix over warps + the tile's global offset
-    for (int d = threadIdx.x; d < kRadix; d += kSortThreads) {
-        uint32_t run = tile_offset[(size_t)d * n_tiles + blockIdx.x];
+
+    // per digit (two per thread): exclusive prefix over warps, tile total
+    const int d0 = 2 * tid;
+    uint32_t tot[kDig] = {0u, 0u};
 #pragma unroll
-        for (int k = 0; k < kWarps; ++k) {
-            uint32_t t = s_cnt[k * kRadix + d];
-            s_cnt[k * kRadix + d] = run;
-            run += t;
+    for (int k = 0; k < kWarps; ++k) {
+        uint2* q = reinterpret_cast<uint2*>(&s_cnt[k * kRadix + d0]);
+        const uint2 v = *q;
+        *q = make_uint2(tot[0], tot[1]);
+        tot[0] += v.x;
+        tot[1] += v.y;
+    }
+    unsigned long long* my_look = a.look + (size_t)tile * kRadix + d0;
+    const uint32_t first_flag = (tile == 0) ? kFlagIncl : kFlagAgg;
+    look_store(my_look, look_pack(a.epoch, first_flag, tot[0]));
+    look_store(my_look + 1, look_pack(a.epoch, first_flag, tot[1]));
+    // block-wide exclusive scan of the digit totals -> first tile-sorted slot of each digit
+    uint32_t x = tot[0] + tot[1];
+    const uint32_t mine = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, o);
+        if (l >= o) x += y;
+    }
+    if (l == 31) s_wsum[w] = x;
+    __syncthreads();
+    uint32_t tstart = x - mine;
+#pragma unroll
+    for (int k = 0; k < kWarps; ++k)
+        if (k < w) tstart += s_wsum[k];
+    // decoupled look-back, both digits in flight together
+    uint32_t excl[kDig] = {0u, 0u};
+    if (tile > 0) {
+        uint32_t j[kDig] = {tile - 1, tile - 1};
+        bool done[kDig] = {false, false};
+        const uint32_t want = a.epoch;
+        while (!(done[0] && done[1])) {
+            unsigned long long v[kDig];
+#pragma unroll
+            for (int q = 0; q < kDig; ++q)
+                if (!done[q]) v[q] = look_load(a.look + (size_t)j[q] * kRadix + d0 + q);
+#pragma unroll
+            for (int q = 0; q < kDig; ++q) {
+                if (done[q]) continue;
+                const uint32_t tag = (uint32_t)(v[q] >> 32);
+                if ((tag >> 2) != want) continue;  // not written yet in this pass
+                excl[q] += (uint32_t)v[q];
+                if ((tag & 3u) == kFlagIncl) done[q] = true;
+                else --j[q];                       // tile 0 always publishes INCLUSIVE, so j never passes 0
+            }
+        }
+        look_store(my_look, look_pack(a.epoch, kFlagIncl, excl[0] + tot[0]));
+        look_store(my_look + 1, look_pack(a.epoch, kFlagIncl, excl[1] + tot[1]));
+    }
+    s_tstart[d0] = tstart;
+    s_tstart[d0 + 1] = tstart + tot[0];
+    s_gdst[d0] = __ldg(&a.gbase[d0]) + excl[0] - tstart;
+    s_gdst[d0 + 1] = __ldg(&a.gbase[d0 + 1]) + excl[1] - (tstart + tot[0]);
+    __syncthreads();
+
+    // tile-sorted slot of every pair (the counters now hold the exclusive prefix over warps)
+#pragma unroll
+    for (int r = 0; r < kSortItems; ++r) {
+        const bool valid = base_w + r * 32 + l < a.n;
+        if (valid) {
+            const uint32_t d = (key[r] >> a.shift) & (kRadix - 1);
+            rnk[r] += s_tstart[d] + cnt[d];
+        }
+    }
+    __syncthreads();  // counters are dead: reuse them as the staging area
+    uint32_t* s_key = smem;
+    uint32_t* s_idx = smem + kSortTile;
+#pragma unroll
+    for (int r = 0; r < kSortItems; ++r) {
+        const uint32_t i = base_w + r * 32 + l;
+        if (i < a.n) {
+            s_key[rnk[r]] = key[r];
+            s_idx[rnk[r]] = (MODE == 0) ? i : __ldg(&a.idx_in[i]);
         }
     }
     __syncthreads();
+    const uint32_t tile_base = tile * kSortTile;
+    const uint32_t n_valid = min((uint32_t)kSortTile, a.n - tile_base);
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
-        uint32_t i = base_w + r * 32 + l;
-        if (i < n) {
-            uint32_t dst = cnt[dig[r]] + rnk[r];
-            io.out_key[0][dst] = __ldg(&io.in_key[0][i]);
-            io.out_key[1][dst] = __ldg(&io.in_key[1][i]);
-            io.out_key[2][dst] = __ldg(&io.in_key[2][i]);
-            io.out_idx[dst] = __ldg(&io.in_idx[i]);
+        const uint32_t s = r * kSortThreads + tid;
+        if (s < n_valid) {
+            const uint32_t k = s_key[s];
+            const uint32_t dst = s_gdst[(k >> a.shift) & (kRadix - 1)] + s;
+            if (a.key_out) a.key_out[dst] = k;
+            a.idx_out[dst] = s_idx[s];
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3  Reorder ("moving"): sorted_pos[i] = pos_mass[perm[i]].  Gather of 16-byte records.
+// a3  Reorder ("moving"): sorted_pos[i] = pos_mass[perm[i]], a gather of 16-byte records; the
+// sorted key words are re-derived from the record in flight (12 B more written, nothing more read).
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_reorder(const float4* __restrict__ pos, const uint32_t* __restrict__ perm,
-                                                 uint32_t n, float4* __restrict__ sorted_pos) {
-    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) sorted_pos[i] = __ldg(&pos[__ldg(&perm[i])]);
+                                                 uint32_t n, const Control* __restrict__ ctl,
+                                                 float4* __restrict__ sorted_pos, uint32_t* __restrict__ khi,
+                                                 uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 p = __ldg(&pos[__ldg(&perm[i])]);
+    sorted_pos[i] = p;
+    uint32_t w[3];
+    morton_words(p, ctl->lo[0], ctl->lo[1], ctl->lo[2], ctl->scale, w);
+    klo[i] = w[0];
+    kmid[i] = w[1];
+    khi[i] = w[2];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -301,49 +413,67 @@ cudaError_t stage_bbox(Ctx* c) {
 }
 
 cudaError_t stage_keys(Ctx* c) {
-    k_keys<<<div_up(c->n, 256), 256, 0, c->stream>>>(c->pos_mass, c->n, c->b.ctl, c->b.key[0][0], c->b.key[0][1],
-                                                     c->b.key[0][2], c->b.idx[0]);
+    Buffers& b = c->b;
+    cudaError_t e = cudaMemsetAsync(b.ghist, 0, sizeof(uint32_t) * kSortPasses * kRadix, c->stream);
+    if (e != cudaSuccess) return e;
+    const uint32_t blocks = min(div_up(c->n, kKeysThreads), (uint32_t)(c->num_sms * 2));
+    k_keys<<<blocks, kKeysThreads, 0, c->stream>>>(c->pos_mass, c->n, b.ctl, b.key[0][0], b.key[0][1], b.key[0][2],
+                                                   b.ghist);
     c->launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t stage_sort(Ctx* c) {
     const uint32_t n = c->n;
-    const uint32_t n_tiles = div_up(n, kSortTile);
     Buffers& b = c->b;
-    cudaError_t e = cudaMemsetAsync(b.ghist, 0, sizeof(uint32_t) * kSortPasses * kRadix, c->stream);
-    if (e != cudaSuccess) return e;
-    uint32_t hb = min(div_up(n, 256 * 16), (uint32_t)(c->num_sms * 4));
-    k_sort_ghist<<<hb, 256, 0, c->stream>>>(b.key[0][0], b.key[0][1], b.key[0][2], n, b.ghist);
-    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist);
-    c->launches += 2;
     static bool attr_set = false;
-    const size_t smem = sizeof(uint32_t) * (kSortThreads / 32) * kRadix;
+    const size_t smem = sizeof(uint32_t) * ((kSortThreads / 32) * kRadix + 2 * kRadix);
     if (!attr_set) {
-        e = cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_sort_pass<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_pass<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_pass<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    int cur = 0;
+    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist);
+    c->launches += 1;
+    SortPass a;
+    a.n = n;
+    a.n_tiles = div_up(n, kSortTile);
+    a.look = b.look;
+    a.ticket = &b.ctl->sort_ticket;
+    int cur = 0;  // pass p reads pair buffer cur (p > 0) and writes cur ^ 1; pass 0 writes buffer 0
     for (int p = 0; p < kSortPasses; ++p) {
-        const int word = 2 - p / 3;  // lo word (index 2) first
-        const int shift = kRadixBits * (p % 3);
-        SortIO io;
-        for (int k = 0; k < 3; ++k) { io.in_key[k] = b.key[cur][k]; io.out_key[k] = b.key[cur ^ 1][k]; }
-        io.in_idx = b.idx[cur];
-        io.out_idx = b.idx[cur ^ 1];
-        k_sort_count<<<n_tiles, kSortThreads, 0, c->stream>>>(b.key[cur][word], n, shift, n_tiles, b.tile_count);
-        k_sort_scan<<<kRadix, 256, 0, c->stream>>>(b.tile_count, n_tiles, b.ghist + p * kRadix);
-        k_sort_scatter<<<n_tiles, kSortThreads, smem, c->stream>>>(io, word, shift, n, n_tiles, b.tile_count);
-        c->launches += 3;
-        cur ^= 1;
+        if (c->sort_epoch >= (1u << 30) - 1) {  // 30-bit epoch about to wrap: forget every stale entry
+            cudaError_t e = cudaMemsetAsync(b.look, 0, sizeof(unsigned long long) * (size_t)div_up(c->n_max, kSortTile) * kRadix,
+                                            c->stream);
+            if (e != cudaSuccess) return e;
+            c->sort_epoch = 0;
+        }
+        a.epoch = ++c->sort_epoch;
+        a.shift = kRadixBits * (p % 3);
+        a.gbase = b.ghist + p * kRadix;
+        a.src_word = b.key[0][2 - p / 3];  // load-order word of this phase: lo, mid, hi
+        const int out = (p == 0) ? 0 : (cur ^ 1);
+        a.key_in = b.pair_key[cur];
+        a.idx_in = b.idx[cur];
+        a.key_out = (p == kSortPasses - 1) ? nullptr : b.pair_key[out];
+        a.idx_out = b.idx[out];
+        if (p == 0) k_sort_pass<0><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
+        else if (p % 3 == 0) k_sort_pass<2><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
+        else k_sort_pass<1><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
+        c->launches += 1;
+        cur = out;
     }
-    c->sorted_buf = cur;
+    c->perm = b.idx[cur];
     return cudaGetLastError();
 }
 
 cudaError_t stage_reorder(Ctx* c) {
-    k_reorder<<<div_up(c->n, 256), 256, 0, c->stream>>>(c->pos_mass, c->b.idx[c->sorted_buf], c->n, c->b.sorted_pos);
+    Buffers& b = c->b;
+    k_reorder<<<div_up(c->n, 256), 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos, b.key[1][0],
+                                                        b.key[1][1], b.key[1][2]);
+    c->sorted_buf = 1;
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -445,7 +445,7 @@ cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
     a.mac = b.c_mac;
     a.quad = b.c_quad;
     a.pos = b.sorted_pos;
-    a.perm = b.idx[c->sorted_buf];
+    a.perm = c->perm;
     a.active_list = b.active_list;
     a.g_first = b.g_first;
     a.g_count = b.g_count;
