@@ -17,6 +17,9 @@ constexpr int kRadixBits = 10;             // one 30-bit key word = 3 digits -> 
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kSortPasses = 9;
 constexpr int kSortThreads = 512;
+constexpr int kSortBlocksPerSM = 2;
+constexpr int kLookBatch = 1;              // look-back entries in flight per digit
+constexpr unsigned kLookSleepNs = 200;     // back-off of a look-back chain whose next entry is not published yet
 constexpr int kSortItems = 16;             // pairs per thread per tile
 constexpr int kSortTile = kSortThreads * kSortItems;
 constexpr int kKeysThreads = 512;

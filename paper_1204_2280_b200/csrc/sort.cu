@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ gh
 // One kernel per pass, single sweep with decoupled look-back:
 //   * tiles of kSortTile pairs are handed out by an atomic ticket, so a tile's predecessors have
 //     always started;
-//   * stable in-tile ranking with __match_any_sync and per-warp digit counters (warp w owns a
+//   * stable in-tile ranking with warp ballots and per-warp digit counters (warp w owns a
 //     contiguous run of the tile, round r, lane l  ->  order = (warp, round, lane));
 //   * each tile publishes, per digit, first its own count (AGGREGATE) and, after summing its
 //     predecessors' entries back to the nearest INCLUSIVE one, its inclusive prefix; an entry is one
@@ -232,11 +232,11 @@ __device__ __forceinline__ void look_store(unsigned long long* p, unsigned long 
 // MODE 0: key = src_word[i], idx = i.   MODE 1: key = key_in[i], idx = idx_in[i].
 // MODE 2: idx = idx_in[i], key = src_word[idx].
 template <int MODE>
-__global__ void __launch_bounds__(kSortThreads, 2) k_sort_pass(const SortPass a) {
+__global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(const SortPass a) {
     extern __shared__ __align__(16) uint32_t smem[];
     constexpr int kWarps = kSortThreads / 32;
     constexpr int kDig = kRadix / kSortThreads;      // digits per thread in the per-digit steps
-    static_assert(kDig == 2, "the per-digit steps below handle two digits per thread");
+    struct __align__(4 * kDig) DigVec { uint32_t x[kDig]; };
     uint32_t* s_cnt = smem;                          // [kWarps][kRadix]; later the staging area
     uint32_t* s_tstart = smem + kWarps * kRadix;     // [kRadix] first tile-sorted slot of the digit
     uint32_t* s_gdst = s_tstart + kRadix;            // [kRadix] global slot of tile-sorted slot 0 of the digit
@@ -276,38 +276,57 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_sort_pass(const SortPass a)
             key[r] = (i < a.n) ? __ldg(&src[i]) : 0u;
         }
     }
+    // Ranking: lanes with the same digit elect their lowest lane, which reserves popc(peers) consecutive
+    // ranks in the warp's counter with one shared-memory atomic and broadcasts the old value.  Rounds are
+    // independent instructions (no warp barrier in between), so the 16 match / atomic / shuffle chains
+    // overlap; the atomics of one warp reach the counter in program order, which keeps the ranks stable.
     const uint32_t lt = (1u << l) - 1u;
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
         const bool valid = base_w + r * 32 + l < a.n;
         const uint32_t d = valid ? ((key[r] >> a.shift) & (kRadix - 1)) : (uint32_t)kRadix;  // kRadix = "no key"
-        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, d);
+        // lanes holding the same digit, one ballot per digit bit (MATCH.ANY serialises over the distinct values
+        // of the warp and is several times slower here: 1024 bins make almost every lane distinct)
+        uint32_t peers = __ballot_sync(0xFFFFFFFFu, valid);
+        if (!valid) peers = ~peers;
+#pragma unroll
+        for (int bit = 0; bit < kRadixBits; ++bit) {
+            const bool on = (d >> bit) & 1u;
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, on);
+            peers &= on ? m : ~m;
+        }
+        const int leader = __ffs(peers) - 1;
         uint32_t pre = 0;
-        if (valid) pre = cnt[d];
-        __syncwarp();
-        if (valid && (peers & lt) == 0) cnt[d] = pre + __popc(peers);
-        __syncwarp();
+        if (valid && l == leader) pre = atomicAdd(&cnt[d], (uint32_t)__popc(peers));
+        pre = __shfl_sync(0xFFFFFFFFu, pre, leader);
         rnk[r] = pre + __popc(peers & lt);
     }
     __syncthreads();
 
-    // per digit (two per thread): exclusive prefix over warps, tile total
-    const int d0 = 2 * tid;
-    uint32_t tot[kDig] = {0u, 0u};
+    // per digit (kDig consecutive digits per thread): exclusive prefix over warps, tile total
+    const int d0 = kDig * tid;
+    uint32_t tot[kDig];
+#pragma unroll
+    for (int q = 0; q < kDig; ++q) tot[q] = 0u;
 #pragma unroll
     for (int k = 0; k < kWarps; ++k) {
-        uint2* q = reinterpret_cast<uint2*>(&s_cnt[k * kRadix + d0]);
-        const uint2 v = *q;
-        *q = make_uint2(tot[0], tot[1]);
-        tot[0] += v.x;
-        tot[1] += v.y;
+        DigVec* pv = reinterpret_cast<DigVec*>(&s_cnt[k * kRadix + d0]);
+        DigVec v = *pv, o;
+#pragma unroll
+        for (int q = 0; q < kDig; ++q) {
+            o.x[q] = tot[q];
+            tot[q] += v.x[q];
+        }
+        *pv = o;
     }
     unsigned long long* my_look = a.look + (size_t)tile * kRadix + d0;
     const uint32_t first_flag = (tile == 0) ? kFlagIncl : kFlagAgg;
-    look_store(my_look, look_pack(a.epoch, first_flag, tot[0]));
-    look_store(my_look + 1, look_pack(a.epoch, first_flag, tot[1]));
+#pragma unroll
+    for (int q = 0; q < kDig; ++q) look_store(my_look + q, look_pack(a.epoch, first_flag, tot[q]));
     // block-wide exclusive scan of the digit totals -> first tile-sorted slot of each digit
-    uint32_t x = tot[0] + tot[1];
+    uint32_t x = 0;
+#pragma unroll
+    for (int q = 0; q < kDig; ++q) x += tot[q];
     const uint32_t mine = x;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -320,34 +339,55 @@ __global__ void __launch_bounds__(kSortThreads, 2) k_sort_pass(const SortPass a)
 #pragma unroll
     for (int k = 0; k < kWarps; ++k)
         if (k < w) tstart += s_wsum[k];
-    // decoupled look-back, both digits in flight together
-    uint32_t excl[kDig] = {0u, 0u};
+    // decoupled look-back, all of the thread's digits in flight together
+    uint32_t excl[kDig];
+#pragma unroll
+    for (int q = 0; q < kDig; ++q) excl[q] = 0u;
     if (tile > 0) {
-        uint32_t j[kDig] = {tile - 1, tile - 1};
-        bool done[kDig] = {false, false};
+        uint32_t j[kDig];
+        uint32_t pending = (1u << kDig) - 1u;
+#pragma unroll
+        for (int q = 0; q < kDig; ++q) j[q] = tile - 1;
         const uint32_t want = a.epoch;
-        while (!(done[0] && done[1])) {
-            unsigned long long v[kDig];
+        // kLookBatch predecessors per digit are fetched together and consumed nearest-first: when a whole wave of
+        // tiles publishes its aggregates at the same moment, the inclusive prefixes ripple forward one L2 round
+        // trip per kLookBatch tiles instead of one per tile.
+        while (pending) {
+            bool missed = false;
+            unsigned long long v[kDig][kLookBatch];
 #pragma unroll
             for (int q = 0; q < kDig; ++q)
-                if (!done[q]) v[q] = look_load(a.look + (size_t)j[q] * kRadix + d0 + q);
+#pragma unroll
+                for (int t = 0; t < kLookBatch; ++t)
+                    if ((pending & (1u << q)) && j[q] >= (uint32_t)t)
+                        v[q][t] = look_load(a.look + (size_t)(j[q] - t) * kRadix + d0 + q);
 #pragma unroll
             for (int q = 0; q < kDig; ++q) {
-                if (done[q]) continue;
-                const uint32_t tag = (uint32_t)(v[q] >> 32);
-                if ((tag >> 2) != want) continue;  // not written yet in this pass
-                excl[q] += (uint32_t)v[q];
-                if ((tag & 3u) == kFlagIncl) done[q] = true;
-                else --j[q];                       // tile 0 always publishes INCLUSIVE, so j never passes 0
+                const uint32_t jq = j[q];
+#pragma unroll
+                for (int t = 0; t < kLookBatch; ++t) {
+                    if (!(pending & (1u << q)) || jq < (uint32_t)t || j[q] != jq - t) continue;
+                    const uint32_t tag = (uint32_t)(v[q][t] >> 32);
+                    if ((tag >> 2) != want) {          // not written yet in this pass: retry from here, a little later
+                        if (t == 0) missed = true;
+                        continue;
+                    }
+                    excl[q] += (uint32_t)v[q][t];
+                    if ((tag & 3u) == kFlagIncl) pending &= ~(1u << q);
+                    else --j[q];                       // tile 0 always publishes INCLUSIVE, so j never passes 0
+                }
             }
+            if (missed) __nanosleep(kLookSleepNs);     // keeps a waiting wave from flooding L2 with re-reads
         }
-        look_store(my_look, look_pack(a.epoch, kFlagIncl, excl[0] + tot[0]));
-        look_store(my_look + 1, look_pack(a.epoch, kFlagIncl, excl[1] + tot[1]));
+#pragma unroll
+        for (int q = 0; q < kDig; ++q) look_store(my_look + q, look_pack(a.epoch, kFlagIncl, excl[q] + tot[q]));
     }
-    s_tstart[d0] = tstart;
-    s_tstart[d0 + 1] = tstart + tot[0];
-    s_gdst[d0] = __ldg(&a.gbase[d0]) + excl[0] - tstart;
-    s_gdst[d0 + 1] = __ldg(&a.gbase[d0 + 1]) + excl[1] - (tstart + tot[0]);
+#pragma unroll
+    for (int q = 0; q < kDig; ++q) {
+        s_tstart[d0 + q] = tstart;
+        s_gdst[d0 + q] = __ldg(&a.gbase[d0 + q]) + excl[q] - tstart;
+        tstart += tot[q];
+    }
     __syncthreads();
 
     // tile-sorted slot of every pair (the counters now hold the exclusive prefix over warps)
