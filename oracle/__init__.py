@@ -250,3 +250,67 @@ def full_step(pos_mass, theta, eps, nleaf=16, ncrit=64, group_mode=2, active_mas
     s = build(pos_mass, nleaf, ncrit, group_mode, active_mask, None, group_cell)
     s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
     return s
+
+
+# ---- row f2: KDK leapfrog and diagnostics (oracle/integrator_oracle.cpp, R22-R24) ----------
+
+def _vel4(vel):
+    """float32[n, 4] copy of a velocity array given as [n, 3] or [n, 4]."""
+    v = np.asarray(vel, dtype=np.float32)
+    out = np.zeros((v.shape[0], 4), np.float32)
+    out[:, :3] = v[:, :3]
+    return out
+
+
+def kick(vel4, acc_pot, h, mask=None):
+    """In place: vel4[i, a] = fma(acc_pot[i, a], h, vel4[i, a]) for masked-in particles (R23)."""
+    assert vel4.dtype == np.float32 and vel4.flags.c_contiguous and vel4.shape[1] == 4
+    ap = _f32(acc_pot)
+    m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+    lib().oracle_kick(_p(vel4, C.c_float), _p(ap, C.c_float), C.c_uint32(vel4.shape[0]), C.c_float(h), _p(m, C.c_uint8))
+
+
+def drift(pos_mass, vel4, h):
+    """In place: pos_mass[i, a] = fma(vel4[i, a], h, pos_mass[i, a]), a < 3 (R23)."""
+    assert pos_mass.dtype == np.float32 and pos_mass.flags.c_contiguous and pos_mass.shape[1] == 4
+    v = _f32(vel4)
+    lib().oracle_drift(_p(pos_mass, C.c_float), _p(v, C.c_float), C.c_uint32(pos_mass.shape[0]), C.c_float(h))
+
+
+DIAG_FIELDS = ("K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "M", "Cx", "Cy", "Cz")
+
+
+def diagnostics(pos_mass, vel4, acc_pot):
+    """float64[12] in the order of DIAG_FIELDS (R24)."""
+    pm, v, ap = _f32(pos_mass), _f32(vel4), _f32(acc_pot)
+    out = np.zeros(12, np.float64)
+    lib().oracle_diagnostics(_p(pm, C.c_float), _p(v, C.c_float), _p(ap, C.c_float), C.c_uint32(pm.shape[0]),
+                             _p(out, C.c_double))
+    return out
+
+
+def force_f32(pos_mass, theta, eps, **kw):
+    """One force step; acc/pot in LOAD order rounded to the fp32 record the library returns (ax, ay, az, phi)."""
+    s = full_step(pos_mass, theta, eps, **kw)
+    ap = np.empty((pos_mass.shape[0], 4), np.float64)
+    ap[s.perm, :3] = s.walk.acc
+    ap[s.perm, 3] = s.walk.pot
+    return ap.astype(np.float32)
+
+
+def leapfrog(pos_mass, vel, theta, eps, dt, n_steps, acc_pot=None, **kw):
+    """n_steps KDK steps with a shared time-step and the tree rebuilt every step (R22; BASELINE.json configs[2]).
+
+    Returns (pos_mass, vel4, acc_pot) after the last step; inputs are not modified.  acc_pot, if given, is the
+    force at the initial positions (otherwise it is computed first).
+    """
+    pm = np.array(pos_mass, dtype=np.float32, order="C")
+    v4 = _vel4(vel)
+    ap = force_f32(pm, theta, eps, **kw) if acc_pot is None else _f32(acc_pot).copy()
+    h = np.float32(0.5) * np.float32(dt)
+    for _ in range(n_steps):
+        kick(v4, ap, h)
+        drift(pm, v4, np.float32(dt))
+        ap = force_f32(pm, theta, eps, **kw)
+        kick(v4, ap, h)
+    return pm, v4, ap
