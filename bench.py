@@ -272,7 +272,7 @@ def run_ours(args):
         ms_per_step = total_ms / args.steps
         value = world * n * args.steps / (total_ms * 1e-3)
         e2e_value = world * n * args.steps / (e2e_total_ms * 1e-3)
-        st = {k: float(np.mean([s[k] for s in stage_ms])) for k in stage_ms[0]}
+        st = {k: float(np.mean([s[k] for s in stage_ms])) for k in stage_ms[0] if k != "integrate"}
         walk_ms = st["walk"]
         flop = FLOP_PP * sum_pp + FLOP_PC * sum_pc
         sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0

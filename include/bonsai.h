@@ -42,7 +42,7 @@ extern "C" {
 #define BONSAI_ENOMEM     (-5)  /* workspace smaller than bonsai_workspace_bytes()                        */
 
 #define BONSAI_MAX_LEVEL   30   /* R1: 30 bits per axis, 90-bit Morton key (BASELINE.json north_star)     */
-#define BONSAI_N_STAGES    8
+#define BONSAI_N_STAGES    9
 
 typedef struct bonsai_ctx bonsai_ctx; /* opaque, host memory, owned by the library */
 
@@ -171,9 +171,46 @@ int bonsai_get_counts(bonsai_ctx* ctx, const uint32_t** n_pp_dev, const uint32_t
 /* Totals of the last walk over all sinks: sum of n_pp and of n_pc (R21).  Waits for the stream. */
 int bonsai_get_interaction_totals(bonsai_ctx* ctx, uint64_t* sum_pp, uint64_t* sum_pc);
 
+/* ---- Time integration around the force step (DESIGN.md row f2) ----------------------------------------
+ * The paper integrates with "the block time-step method" (P:L24 Introduction; P:L32 Results: only "particles
+ * that have to be updated" are walked) and states no scheme; BASELINE.json configs[2] fixes leapfrog steps with
+ * a shared time-step and the tree rebuilt every step.  Readings R22 (kick-drift-kick), R23 (fp32 state, each
+ * component updated by ONE fused multiply-add rounded once), R24 (diagnostics) of DESIGN.md.
+ *
+ * All arrays are device, 16-byte aligned float4[n] in LOAD order, caller-owned:
+ *   pos_mass (x, y, z, m)   vel (vx, vy, vz, unused -- carried through)   acc_pot (ax, ay, az, phi) as bonsai_walk
+ *   writes it.  n <= n_max.  Asynchronous on the context's stream.  EINVAL on null / misaligned / n / non-finite step. */
+
+/* Kick: vel[i].xyz = fma(acc_pot[i].xyz, step, vel[i].xyz) for every i whose mask byte is non-zero (all i when
+ * active_mask_dev is NULL; u8[n], load order -- the same mask bonsai_walk takes, R19). */
+int bonsai_kick(bonsai_ctx* ctx, float* vel_dev, const float* acc_pot_dev, uint32_t n, float step,
+                const uint8_t* active_mask_dev);
+
+/* Drift: pos_mass[i].xyz = fma(vel[i].xyz, step, pos_mass[i].xyz); masses untouched; every particle drifts.
+ * If pos_mass_dev is the array given to bonsai_load(), the context falls back to the "loaded" state: the tree no
+ * longer matches the positions and bonsai_build_tree() must run before the next walk (ESTATE otherwise). */
+int bonsai_drift(bonsai_ctx* ctx, float* pos_mass_dev, const float* vel_dev, uint32_t n, float step);
+
+/* One kick-drift-kick step of size dt with a shared time-step (R22):
+ *   vel += acc (dt/2);  pos += vel dt;  [load, build_tree, compute_multipoles, walk(theta, eps, all active)];
+ *   vel += acc_new (dt/2).
+ * On entry acc_pot_dev holds the force at the current positions (from a previous bonsai_walk or
+ * bonsai_leapfrog_step); on return it holds the force at the new positions.  The opening kick and the drift run
+ * as one fused pass with the same arithmetic as bonsai_kick followed by bonsai_drift. */
+int bonsai_leapfrog_step(bonsai_ctx* ctx, float* pos_mass_dev, float* vel_dev, float* acc_pot_dev, uint32_t n,
+                         float theta, float eps, float dt);
+
+/* Diagnostics (R24), fp64 sums of the fp32 state, G = 1; writes 12 doubles to out12_dev (device, 8-byte aligned):
+ *   [0] K = 1/2 sum m |v|^2   [1] W = 1/2 sum m phi   [2..4] P = sum m v   [5..7] L = sum m (x cross v)
+ *   [8] M = sum m             [9..11] C = sum m x.
+ * Deterministic for a given n (fixed reduction tree). */
+int bonsai_diagnostics(bonsai_ctx* ctx, const float* pos_mass_dev, const float* vel_dev, const float* acc_pot_dev,
+                       uint32_t n, double* out12_dev);
+
 /* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events between stages from then on;
  * bonsai_get_stage_ms() waits for the stream and writes milliseconds of the most recent execution of each
- * stage: 0 bbox, 1 keys, 2 sort, 3 reorder, 4 build, 5 groups, 6 multipoles, 7 walk. */
+ * stage: 0 bbox, 1 keys, 2 sort, 3 reorder, 4 build, 5 groups, 6 multipoles, 7 walk, 8 integrate (the most
+ * recent kick / drift / kick+drift launch). */
 int bonsai_set_timing(bonsai_ctx* ctx, int enable);
 int bonsai_get_stage_ms(bonsai_ctx* ctx, float out_ms[BONSAI_N_STAGES]);
 

@@ -18,8 +18,9 @@ import torch
 from . import build as _build
 
 OK, EINVAL, ESTATE, ECAPACITY, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
-N_STAGES = 8
-STAGES = ("bbox", "keys", "sort", "reorder", "build", "groups", "multipoles", "walk")
+N_STAGES = 9
+STAGES = ("bbox", "keys", "sort", "reorder", "build", "groups", "multipoles", "walk", "integrate")
+DIAG_FIELDS = ("K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "M", "Cx", "Cy", "Cz")
 
 # every symbol include/bonsai.h declares (tests check the library exports exactly these)
 SYMBOLS = (
@@ -28,6 +29,7 @@ SYMBOLS = (
     "bonsai_get_keys", "bonsai_get_perm", "bonsai_get_sorted_pos", "bonsai_get_cells", "bonsai_get_groups",
     "bonsai_get_counts", "bonsai_get_interaction_totals", "bonsai_set_timing", "bonsai_get_stage_ms",
     "bonsai_get_launch_count", "bonsai_strerror",
+    "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics",
 )
 
 
@@ -86,6 +88,10 @@ def lib() -> C.CDLL:
     L.bonsai_get_stage_ms.argtypes = [vp, C.POINTER(f32)]
     L.bonsai_get_launch_count.argtypes = [vp]
     L.bonsai_get_launch_count.restype = C.c_uint64
+    L.bonsai_kick.argtypes = [vp, vp, vp, u32, f32, vp]
+    L.bonsai_drift.argtypes = [vp, vp, vp, u32, f32]
+    L.bonsai_leapfrog_step.argtypes = [vp, vp, vp, vp, u32, f32, f32, f32]
+    L.bonsai_diagnostics.argtypes = [vp, vp, vp, vp, u32, vp]
     L.bonsai_strerror.argtypes = [C.c_int]
     L.bonsai_strerror.restype = C.c_char_p
     for name in SYMBOLS:  # fail loudly on a stale or partial library
@@ -231,6 +237,50 @@ class Bonsai:
                                             out_host.data_ptr()), "bonsai_step_host")
         self.n = n
         return out_host
+
+    # ---- row f2: integrator and diagnostics ---------------------------------------------------------
+    def _f4(self, t: torch.Tensor, n: int | None = None) -> int:
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.dim() == 2 and t.shape[1] == 4
+        assert n is None or t.shape[0] == n
+        return t.data_ptr()
+
+    def kick(self, vel: torch.Tensor, acc_pot: torch.Tensor, step: float, active_mask: torch.Tensor | None = None) -> None:
+        """In place on the device: vel.xyz = fma(acc_pot.xyz, step, vel.xyz) for masked-in particles (float32[n,4])."""
+        n = vel.shape[0]
+        mptr = None
+        if active_mask is not None:
+            assert active_mask.is_cuda and active_mask.dtype == torch.uint8 and active_mask.numel() == n
+            mptr = active_mask.data_ptr()
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_kick(self._h, self._f4(vel), self._f4(acc_pot, n), n, float(step), mptr), "bonsai_kick")
+
+    def drift(self, pos_mass: torch.Tensor, vel: torch.Tensor, step: float) -> None:
+        """In place on the device: pos_mass.xyz = fma(vel.xyz, step, pos_mass.xyz)."""
+        n = pos_mass.shape[0]
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_drift(self._h, self._f4(pos_mass), self._f4(vel, n), n, float(step)), "bonsai_drift")
+
+    def leapfrog_step(self, pos_mass: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor, theta: float,
+                      eps: float, dt: float) -> None:
+        """One KDK step in place (bonsai_leapfrog_step); acc_pot is the force at the current positions on entry."""
+        n = pos_mass.shape[0]
+        self._keep = [pos_mass]
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_leapfrog_step(self._h, self._f4(pos_mass), self._f4(vel, n), self._f4(acc_pot, n), n,
+                                                float(theta), float(eps), float(dt)), "bonsai_leapfrog_step")
+        self.n = n
+
+    def diagnostics(self, pos_mass: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor,
+                    out: torch.Tensor | None = None) -> torch.Tensor:
+        """float64[12] device tensor in the order of DIAG_FIELDS (asynchronous)."""
+        n = pos_mass.shape[0]
+        if out is None:
+            out = torch.zeros(12, dtype=torch.float64, device=self.device)
+        assert out.is_cuda and out.dtype == torch.float64 and out.numel() == 12 and out.is_contiguous()
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_diagnostics(self._h, self._f4(pos_mass), self._f4(vel, n), self._f4(acc_pot, n), n,
+                                              out.data_ptr()), "bonsai_diagnostics")
+        return out
 
     def sync(self) -> None:
         _check(self._L.bonsai_sync(self._h), "bonsai_sync")

@@ -98,6 +98,7 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     t.scan_tmp = cv.take<uint32_t>((size_t)div_up(n + 1, 2048) + 2);
     t.n_pp = cv.take<uint32_t>(n);
     t.n_pc = cv.take<uint32_t>(n);
+    t.diag_partial = cv.take<double>((size_t)kDiagMaxBlocks * 12);
     t.host_in = cv.take<float4>(n);
     t.host_out = cv.take<float4>(n);
     t.host_mask = cv.take<uint8_t>(n);
@@ -251,6 +252,71 @@ int bonsai_step_host(bonsai_ctx* h, const float* pos_mass_host, uint32_t n, floa
                           reinterpret_cast<float*>(b.host_out))) != BONSAI_OK) return rc;
     BONSAI_TRY(cudaMemcpyAsync(acc_pot_host_out, b.host_out, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
     return bonsai_sync(h);
+}
+
+
+// ---- row f2: integrator and diagnostics (integrate.cu) --------------------------------------------
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) % 16) == 0; }
+
+int bonsai_kick(bonsai_ctx* h, float* vel_dev, const float* acc_pot_dev, uint32_t n, float step,
+                const uint8_t* active_mask_dev) {
+    if (!h || !vel_dev || !acc_pot_dev || !aligned16(vel_dev) || !aligned16(acc_pot_dev)) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max || !std::isfinite(step)) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    StageTimer t(c, 8);
+    BONSAI_TRY(stage_kick(c, reinterpret_cast<float4*>(vel_dev), reinterpret_cast<const float4*>(acc_pot_dev), n, step,
+                          active_mask_dev));
+    return BONSAI_OK;
+}
+
+int bonsai_drift(bonsai_ctx* h, float* pos_mass_dev, const float* vel_dev, uint32_t n, float step) {
+    if (!h || !pos_mass_dev || !vel_dev || !aligned16(pos_mass_dev) || !aligned16(vel_dev)) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max || !std::isfinite(step)) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    StageTimer t(c, 8);
+    BONSAI_TRY(stage_drift(c, reinterpret_cast<float4*>(pos_mass_dev), reinterpret_cast<const float4*>(vel_dev), n, step));
+    if (c->pos_mass == reinterpret_cast<const float4*>(pos_mass_dev) && c->state > 1) c->state = 1;  // the tree is stale
+    return BONSAI_OK;
+}
+
+int bonsai_diagnostics(bonsai_ctx* h, const float* pos_mass_dev, const float* vel_dev, const float* acc_pot_dev,
+                       uint32_t n, double* out12_dev) {
+    if (!h || !pos_mass_dev || !vel_dev || !acc_pot_dev || !out12_dev) return BONSAI_EINVAL;
+    if (!aligned16(pos_mass_dev) || !aligned16(vel_dev) || !aligned16(acc_pot_dev) ||
+        (reinterpret_cast<uintptr_t>(out12_dev) % 8) != 0)
+        return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    BONSAI_TRY(stage_diagnostics(c, reinterpret_cast<const float4*>(pos_mass_dev), reinterpret_cast<const float4*>(vel_dev),
+                                 reinterpret_cast<const float4*>(acc_pot_dev), n, out12_dev));
+    return BONSAI_OK;
+}
+
+int bonsai_leapfrog_step(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, float* acc_pot_dev, uint32_t n, float theta,
+                         float eps, float dt) {
+    if (!h || !pos_mass_dev || !vel_dev || !acc_pot_dev) return BONSAI_EINVAL;
+    if (!aligned16(pos_mass_dev) || !aligned16(vel_dev) || !aligned16(acc_pot_dev)) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max || !std::isfinite(dt)) return BONSAI_EINVAL;
+    if (!(theta >= 0.0f) || !(eps >= 0.0f) || std::isinf(theta) || std::isinf(eps)) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    const float half = 0.5f * dt;  // exact
+    {
+        StageTimer t(c, 8);
+        BONSAI_TRY(stage_kick_drift(c, reinterpret_cast<float4*>(pos_mass_dev), reinterpret_cast<float4*>(vel_dev),
+                                    reinterpret_cast<const float4*>(acc_pot_dev), n, half, dt));
+    }
+    int rc;
+    if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_walk(h, theta, eps, nullptr, acc_pot_dev)) != BONSAI_OK) return rc;
+    {
+        StageTimer t(c, 8);
+        BONSAI_TRY(stage_kick(c, reinterpret_cast<float4*>(vel_dev), reinterpret_cast<const float4*>(acc_pot_dev), n, half,
+                              nullptr));
+    }
+    return BONSAI_OK;
 }
 
 void bonsai_destroy(bonsai_ctx* h) {

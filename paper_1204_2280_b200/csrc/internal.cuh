@@ -31,6 +31,9 @@ constexpr int kTreeTile = kTreeThreads * kTreeItems;  // particles per block
 constexpr int kLevelSlots = 32;                       // levels 0..30, padded
 constexpr int kMaxNleaf = 64;
 
+// ---- diagnostics (integrate.cu) ----------------------------------------------------------------
+constexpr int kDiagMaxBlocks = 1184;       // 8 blocks per SM on 148 SMs
+
 // ---- walk geometry (walk.cu) -------------------------------------------------------------------
 constexpr int kWalkWarps = 8;              // warps per block, one group per warp at a time
 constexpr int kWalkStack = 512;            // traversal stack entries per warp (see walk.cu for the bound)
@@ -50,7 +53,7 @@ struct Control {
     uint32_t walk_ticket;      // dynamic group scheduler of the walk
     uint32_t level_ticket;     // last-block-done counter of k_tree_scan_levels
     uint32_t sort_ticket;      // tile scheduler of k_sort_pass (reset by the tile that draws the last ticket)
-    uint32_t pad0[1];
+    uint32_t diag_ticket;      // last-block-done counter of k_diagnostics
     uint32_t level_offsets[32];  // first cell of level L; [31] = n_cells
     unsigned long long sum_pp;   // interaction totals of the last walk (sink-source pairs)
     unsigned long long sum_pc;
@@ -108,6 +111,7 @@ struct Buffers {
     uint32_t* scan_tmp;        // block sums of the device-wide scan
     // walk
     uint32_t *n_pp, *n_pc;     // [n] load order
+    double* diag_partial;      // [kDiagMaxBlocks][12] block partials of k_diagnostics
     // staging of bonsai_step_host
     float4 *host_in, *host_out;
     uint8_t* host_mask;
@@ -144,6 +148,10 @@ cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order);
 cudaError_t stage_multipoles(Ctx* c);
 cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out);
 size_t walk_smem_bytes(uint32_t nleaf);
+cudaError_t stage_kick(Ctx* c, float4* vel, const float4* acc, uint32_t n, float h, const uint8_t* mask);
+cudaError_t stage_drift(Ctx* c, float4* pos, const float4* vel, uint32_t n, float h);
+cudaError_t stage_kick_drift(Ctx* c, float4* pos, float4* vel, const float4* acc, uint32_t n, float hk, float hd);
+cudaError_t stage_diagnostics(Ctx* c, const float4* pos, const float4* vel, const float4* acc, uint32_t n, double* out);
 
 // Device-wide exclusive scan of u32 (scan.cu): out[i] = sum_{j<i} in[j], i in [0, n]; out has n+1 entries
 // (out[n] = total).  in may alias out.  tmp needs div_up(n, 2048) + 1 entries.
