@@ -314,3 +314,32 @@ def leapfrog(pos_mass, vel, theta, eps, dt, n_steps, acc_pot=None, **kw):
         ap = force_f32(pm, theta, eps, **kw)
         kick(v4, ap, h)
     return pm, v4, ap
+
+
+# ---- row f1: refreshed tree (oracle/refresh_oracle.cpp, R25) --------------------------------
+
+def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, group_cell=1024) -> Step:
+    """The structures of ``prev`` (permutation, keys, cells, group membership) carried over to moved particles.
+
+    pos_mass is the SAME particles in the SAME load order as the build that produced ``prev``.
+    """
+    del nleaf  # the cells are frozen
+    import copy
+    pm = _f32(pos_mass)
+    spm = np.ascontiguousarray(pm[prev.perm])
+    t = copy.deepcopy(prev.tree)
+    act_sorted = None if active_mask is None else np.ascontiguousarray(active_mask, np.uint8)[prev.perm]
+    g = groups(group_mode, ncrit, spm, t, act_sorted, group_cell)
+    multipoles(spm, prev.sorted_keys, prev.lo, prev.side, t)
+    lo = _f32(prev.lo)
+    sk = np.ascontiguousarray(prev.sorted_keys, dtype=np.uint32)
+    lib().oracle_extent_side(_p(spm, C.c_float), _p(sk, C.c_uint32), _p(lo, C.c_float), C.c_double(prev.side),
+                             C.c_uint32(t.n_cells), _p(t.level, C.c_uint32), _p(t.first, C.c_uint32),
+                             _p(t.count, C.c_uint32), _p(t.lside, C.c_float))
+    return Step(prev.lo, prev.side, prev.keys, prev.perm, spm, prev.sorted_keys, t, g)
+
+
+def refreshed_step(prev: Step, pos_mass, theta, eps, sel=None, **kw) -> Step:
+    s = refresh(prev, pos_mass, **kw)
+    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
+    return s

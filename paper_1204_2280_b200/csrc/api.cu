@@ -86,6 +86,7 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     t.c_qraw = cv.take<float>(cap * 6);
     t.c_mom = cv.take<double>(cap * 10);
     t.c_arrived = cv.take<uint32_t>(cap);
+    t.c_box = cv.take<float>(cap * 6);
     t.rank = cv.take<uint32_t>((size_t)n + 1);
     t.active_list = cv.take<uint32_t>(n);
     t.g_flag = cv.take<uint32_t>((size_t)n + 1);
@@ -159,6 +160,8 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.sort_epoch = 0;
     c.state = 0;
     c.groups_all_active = false;
+    c.tree_valid = false;
+    c.tree_refreshed = false;
     c.timing = false;
     c.launches = 0;
     for (int s = 0; s < BONSAI_N_STAGES; ++s) {
@@ -174,9 +177,9 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     // control block, the self-cleaning arrival counters and the sort's look-back table (epoch 0 = never written)
     // start at zero
     if (cudaMemsetAsync(c.b.ctl, 0, sizeof(Control), c.stream) != cudaSuccess ||
+        cudaMemsetAsync(c.b.c_arrived, 0, sizeof(uint32_t) * (size_t)c.cap_cells, c.stream) != cudaSuccess ||
         cudaMemsetAsync(c.b.look, 0, sizeof(unsigned long long) * (size_t)kRadix * div_up(n_max, kSortTile), c.stream) !=
-            cudaSuccess ||
-        cudaMemsetAsync(c.b.c_arrived, 0, sizeof(uint32_t) * (size_t)c.cap_cells, c.stream) != cudaSuccess) {
+            cudaSuccess) {
         delete h;
         return BONSAI_ECUDA;
     }

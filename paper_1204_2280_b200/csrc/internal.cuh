@@ -54,6 +54,7 @@ struct Control {
     uint32_t level_ticket;     // last-block-done counter of k_tree_scan_levels
     uint32_t sort_ticket;      // tile scheduler of k_sort_pass (reset by the tile that draws the last ticket)
     uint32_t diag_ticket;      // last-block-done counter of k_diagnostics
+    uint32_t pad1[4];
     uint32_t level_offsets[32];  // first cell of level L; [31] = n_cells
     unsigned long long sum_pp;   // interaction totals of the last walk (sink-source pairs)
     unsigned long long sum_pc;
@@ -101,6 +102,7 @@ struct Buffers {
     float* c_qraw;             // [cap][6] raw second moments xx, yy, zz, xy, xz, yz as fp32 (introspection, R8)
     double* c_mom;             // [cap][10] fp64: M, COMx, COMy, COMz, Qxx, Qyy, Qzz, Qxy, Qxz, Qyz
     uint32_t* c_arrived;       // [cap] children that have finished
+    float* c_box;              // [cap][6] exact fp32 bounding box of each cell's members (min xyz, max xyz)
     // groups
     uint32_t* rank;            // [n+1] exclusive count of active particles (sorted order)
     uint32_t* active_list;     // [n]
@@ -129,6 +131,8 @@ struct Ctx {
     uint32_t sort_epoch;       // tag of the last k_sort_pass launch (30 bits, see sort.cu)
     int state;                 // 0 created, 1 loaded, 2 tree built, 3 multipoles done, 4 walked
     bool groups_all_active;    // the group list on the device is the all-active one
+    bool tree_valid;           // a tree for the current n exists (bonsai_refresh_tree may reuse it)
+    bool tree_refreshed;       // positions were re-gathered into a frozen tree: multipoles take l from the extents (R25)
     bool timing;
     cudaEvent_t ev[BONSAI_N_STAGES][2];
     bool ev_valid[BONSAI_N_STAGES];
