@@ -171,6 +171,19 @@ int bonsai_get_counts(bonsai_ctx* ctx, const uint32_t** n_pp_dev, const uint32_t
 /* Totals of the last walk over all sinks: sum of n_pp and of n_pc (R21).  Waits for the stream. */
 int bonsai_get_interaction_totals(bonsai_ctx* ctx, uint64_t* sum_pp, uint64_t* sum_pc);
 
+/* Re-use the sorted order and the tree of the last bonsai_build_tree() after the particles have moved (P:L52:
+ * sorting, moving and tree-construction "do not have to be executed during each time-step when using the block
+ * time-step method. It is sufficient to only recompute the multipole moments ..."; reading R25 of DESIGN.md).
+ * The array given to bonsai_load() must hold the SAME particles in the SAME load order as at the last build, with
+ * new positions (e.g. after bonsai_drift()).  Keeps permutation, keys, cells, links, geometric centres and group
+ * membership; re-gathers the particles into sorted order and recomputes the group boxes.  The next
+ * bonsai_compute_multipoles() then recomputes every moment from the new positions and lets the cell side that
+ * enters the opening test grow to the extent of the cell's members:
+ *     l' = max(l, 2 max_i max_a |x_ia - g_a|)   (fp64, rounded once).
+ * Forces stay valid Barnes-Hut forces for the new positions; the interaction count grows with the drift, and the
+ * caller decides when to rebuild (bonsai_get_interaction_totals()).  ESTATE when no tree for this n exists. */
+int bonsai_refresh_tree(bonsai_ctx* ctx);
+
 /* ---- Time integration around the force step (DESIGN.md row f2) ----------------------------------------
  * The paper integrates with "the block time-step method" (P:L24 Introduction; P:L32 Results: only "particles
  * that have to be updated" are walked) and states no scheme; BASELINE.json configs[2] fixes leapfrog steps with

@@ -29,7 +29,7 @@ SYMBOLS = (
     "bonsai_get_keys", "bonsai_get_perm", "bonsai_get_sorted_pos", "bonsai_get_cells", "bonsai_get_groups",
     "bonsai_get_counts", "bonsai_get_interaction_totals", "bonsai_set_timing", "bonsai_get_stage_ms",
     "bonsai_get_launch_count", "bonsai_strerror",
-    "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics",
+    "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
 )
 
 
@@ -88,6 +88,7 @@ def lib() -> C.CDLL:
     L.bonsai_get_stage_ms.argtypes = [vp, C.POINTER(f32)]
     L.bonsai_get_launch_count.argtypes = [vp]
     L.bonsai_get_launch_count.restype = C.c_uint64
+    L.bonsai_refresh_tree.argtypes = [vp]
     L.bonsai_kick.argtypes = [vp, vp, vp, u32, f32, vp]
     L.bonsai_drift.argtypes = [vp, vp, vp, u32, f32]
     L.bonsai_leapfrog_step.argtypes = [vp, vp, vp, vp, u32, f32, f32, f32]
@@ -192,6 +193,10 @@ class Bonsai:
     def build_tree(self) -> None:
         with torch.cuda.device(self.device):
             _check(self._L.bonsai_build_tree(self._h), "bonsai_build_tree")
+
+    def refresh_tree(self) -> None:
+        """Keep the sorted order and the cells of the last build_tree(); re-gather the moved particles (R25)."""
+        _check(self._L.bonsai_refresh_tree(self._h), "bonsai_refresh_tree")
 
     def compute_multipoles(self) -> None:
         with torch.cuda.device(self.device):

@@ -160,7 +160,7 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.sort_epoch = 0;
     c.state = 0;
     c.groups_all_active = false;
-    c.tree_valid = false;
+    c.tree_n = 0;
     c.tree_refreshed = false;
     c.timing = false;
     c.launches = 0;
@@ -204,9 +204,22 @@ int bonsai_build_tree(bonsai_ctx* h) {
     { StageTimer t(c, 0); BONSAI_TRY(stage_bbox(c)); }
     { StageTimer t(c, 1); BONSAI_TRY(stage_keys(c)); }
     { StageTimer t(c, 2); BONSAI_TRY(stage_sort(c)); }
-    { StageTimer t(c, 3); BONSAI_TRY(stage_reorder(c)); }
+    { StageTimer t(c, 3); BONSAI_TRY(stage_reorder(c, true)); }
     { StageTimer t(c, 4); BONSAI_TRY(stage_build(c)); }
     { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
+    c->tree_n = c->n;
+    c->tree_refreshed = false;
+    c->state = 2;
+    return BONSAI_OK;
+}
+
+int bonsai_refresh_tree(bonsai_ctx* h) {
+    if (!h) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    if (c->state < 1 || c->tree_n == 0 || c->tree_n != c->n) return BONSAI_ESTATE;
+    { StageTimer t(c, 3); BONSAI_TRY(stage_reorder(c, false)); }
+    { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
+    c->tree_refreshed = true;
     c->state = 2;
     return BONSAI_OK;
 }

@@ -131,7 +131,7 @@ struct Ctx {
     uint32_t sort_epoch;       // tag of the last k_sort_pass launch (30 bits, see sort.cu)
     int state;                 // 0 created, 1 loaded, 2 tree built, 3 multipoles done, 4 walked
     bool groups_all_active;    // the group list on the device is the all-active one
-    bool tree_valid;           // a tree for the current n exists (bonsai_refresh_tree may reuse it)
+    uint32_t tree_n;           // particle count of the tree on the device (0 = none): bonsai_refresh_tree may reuse it
     bool tree_refreshed;       // positions were re-gathered into a frozen tree: multipoles take l from the extents (R25)
     bool timing;
     cudaEvent_t ev[BONSAI_N_STAGES][2];
@@ -146,7 +146,7 @@ inline uint32_t div_up(uint32_t a, uint32_t b) { return (a + b - 1) / b; }
 cudaError_t stage_bbox(Ctx* c);
 cudaError_t stage_keys(Ctx* c);
 cudaError_t stage_sort(Ctx* c);
-cudaError_t stage_reorder(Ctx* c);
+cudaError_t stage_reorder(Ctx* c, bool write_keys);
 cudaError_t stage_build(Ctx* c);
 cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order);
 cudaError_t stage_multipoles(Ctx* c);

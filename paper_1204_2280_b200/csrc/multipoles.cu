@@ -30,7 +30,8 @@ struct Mom {
     double m, cx, cy, cz, xx, yy, zz, xy, xz, yz;
 };
 
-__device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], const float (&mx)[3], int use_extent,
+template <bool use_extent>
+__device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], const float (&mx)[3],
                                            uint32_t c, int L, uint32_t khi, uint32_t kmid, uint32_t klo,
                                            const Control* __restrict__ ctl, uint32_t link_first, uint32_t link_info,
                                            double* __restrict__ c_mom, float* __restrict__ c_box,
@@ -46,13 +47,11 @@ __device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], c
         const uint32_t ca = (L == 0) ? 0u : (qa >> (kMaxLevel - L));
         g[a] = __dadd_rn((double)ctl->lo[a], __dmul_rn(__dadd_rn((double)ca, 0.5), l));
     }
-    float* bx = c_box + (size_t)c * 6;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        __stcg(&bx[d], mn[d]);
-        __stcg(&bx[3 + d], mx[d]);
-    }
     if (use_extent) {
+        float2* bx = reinterpret_cast<float2*>(c_box + (size_t)c * 6);  // only a refreshed tree needs the boxes
+        __stcg(&bx[0], make_float2(mn[0], mn[1]));
+        __stcg(&bx[1], make_float2(mn[2], mx[0]));
+        __stcg(&bx[2], make_float2(mx[1], mx[2]));
         // R25 (refreshed tree): the side becomes the side of the smallest cube about the geometric centre that
         // holds every member, never less than the geometric side: l = max(l, 2 max_axis max(g - min, max - g)), fp64
         double e = 0.0;
@@ -94,8 +93,8 @@ struct TreeView {
     const uint32_t *level, *first, *count, *first_child, *n_child, *parent;
 };
 
-__global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ ctl, uint32_t cap_cells, int use_extent,
-                                                    TreeView t,
+template <bool use_extent>
+__global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ ctl, uint32_t cap_cells, TreeView t,
                                                     const float4* __restrict__ sorted_pos,
                                                     const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
                                                     const uint32_t* __restrict__ klo, double* __restrict__ c_mom,
@@ -114,9 +113,11 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         for (uint32_t k = 0; k < cnt; ++k) {
             const float4 p = __ldg(&sorted_pos[f + k]);
             const double m = (double)p.w;
-            mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
-            mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
-            mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
+            if (use_extent) {
+                mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
+                mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
+                mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
+            }
             q.m = __dadd_rn(q.m, m);
             sx = __dadd_rn(sx, __dmul_rn(m, (double)p.x));
             sy = __dadd_rn(sy, __dmul_rn(m, (double)p.y));
@@ -139,7 +140,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
                 q.yz = __dadd_rn(q.yz, __dmul_rn(__dmul_rn(m, dy), dz));
             }
         }
-        store_cell(q, mn, mx, use_extent, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f,
+        store_cell<use_extent>(q, mn, mx, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f,
                    kLeafBit | cnt, c_mom, c_box, c_mac, c_quad, c_qraw);
     }
     for (;;) {
@@ -157,11 +158,11 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         q.m = 0.0;
         for (uint32_t k = 0; k < nc; ++k) {
             const double* mo = c_mom + (size_t)(fc + k) * 10;
-            const float* bx = c_box + (size_t)(fc + k) * 6;
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                mn[d] = fminf(mn[d], __ldcg(&bx[d]));
-                mx[d] = fmaxf(mx[d], __ldcg(&bx[3 + d]));
+            if (use_extent) {
+                const float2* bx = reinterpret_cast<const float2*>(c_box + (size_t)(fc + k) * 6);
+                const float2 b0 = __ldcg(&bx[0]), b1 = __ldcg(&bx[1]), b2 = __ldcg(&bx[2]);
+                mn[0] = fminf(mn[0], b0.x); mn[1] = fminf(mn[1], b0.y); mn[2] = fminf(mn[2], b1.x);
+                mx[0] = fmaxf(mx[0], b1.y); mx[1] = fmaxf(mx[1], b2.x); mx[2] = fmaxf(mx[2], b2.y);
             }
             const double m = __ldcg(&mo[0]);
             q.m += m;
@@ -187,7 +188,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
             }
         }
         const uint32_t f = t.first[p];
-        store_cell(q, mn, mx, use_extent, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc,
+        store_cell<use_extent>(q, mn, mx, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc,
                    c_mom, c_box, c_mac, c_quad, c_qraw);
         c = p;
     }
@@ -197,10 +198,15 @@ cudaError_t stage_multipoles(Ctx* c) {
     Buffers& b = c->b;
     const int s = c->sorted_buf;
     TreeView t{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
-    k_multipoles<<<div_up(c->cap_cells, 128), 128, 0, c->stream>>>(b.ctl, c->cap_cells, c->tree_refreshed ? 1 : 0, t,
-                                                                   b.sorted_pos, b.key[s][0], b.key[s][1], b.key[s][2],
-                                                                   b.c_mom, b.c_mac, b.c_quad, b.c_qraw, b.c_box,
-                                                                   b.c_arrived);
+    const dim3 grid(div_up(c->cap_cells, 128));
+    if (c->tree_refreshed)
+        k_multipoles<true><<<grid, 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1],
+                                                        b.key[s][2], b.c_mom, b.c_mac, b.c_quad, b.c_qraw, b.c_box,
+                                                        b.c_arrived);
+    else
+        k_multipoles<false><<<grid, 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1],
+                                                         b.key[s][2], b.c_mom, b.c_mac, b.c_quad, b.c_qraw, b.c_box,
+                                                         b.c_arrived);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -437,6 +437,7 @@ __global__ void __launch_bounds__(256) k_reorder(const float4* __restrict__ pos,
     if (i >= n) return;
     const float4 p = __ldg(&pos[__ldg(&perm[i])]);
     sorted_pos[i] = p;
+    if (khi == nullptr) return;  // refresh of a frozen tree (R25): the keys stay those of the last build
     uint32_t w[3];
     morton_words(p, ctl->lo[0], ctl->lo[1], ctl->lo[2], ctl->scale, w);
     klo[i] = w[0];
@@ -509,10 +510,10 @@ cudaError_t stage_sort(Ctx* c) {
     return cudaGetLastError();
 }
 
-cudaError_t stage_reorder(Ctx* c) {
+cudaError_t stage_reorder(Ctx* c, bool write_keys) {
     Buffers& b = c->b;
-    k_reorder<<<div_up(c->n, 256), 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos, b.key[1][0],
-                                                        b.key[1][1], b.key[1][2]);
+    k_reorder<<<div_up(c->n, 256), 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos,
+                                                        write_keys ? b.key[1][0] : nullptr, b.key[1][1], b.key[1][2]);
     c->sorted_buf = 1;
     c->launches += 1;
     return cudaGetLastError();
