@@ -282,7 +282,9 @@ def run_ours(args):
         hbm = peaks.get("hbm_gbs", 6650.0)
         hbm_src = "measured" if "hbm_gbs" in peaks else "fallback"
         # algorithmic bytes per particle of the HBM-bound stages
-        alg_bytes = {"bbox": 16, "keys": 32, "sort": 12 + 9 * 32, "reorder": 36, "groups": 16 + 24 / args.ncrit}
+        # keys: 16 in + 3 words out; sort: 9 pair passes x (8 in + 8 out), minus the index read of pass 0 (iota) and
+        # the key write of pass 8; reorder: perm + record in, record + 3 key words out
+        alg_bytes = {"bbox": 16, "keys": 28, "sort": 9 * 16 - 8, "reorder": 48, "groups": 16 + 24 / args.ncrit}
         stages = {}
         for k, v in st.items():
             ent = {"ms": v, "share": v / sum(st.values())}
@@ -303,7 +305,7 @@ def run_ours(args):
                     "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n},
             "gpu_launches": int(launches),
             "roofline": {"kernel": "k_walk", "bound": "alu", "achieved": achieved_tf, "peak": peak_tf,
-                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": walk_traffic(args),
                          "peak_source": f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x "
                                         f"{sm_max:.0f} MHz (clocks.max.sm); no fp32 entry in MEASURED_PEAKS.json",
                          "flop_convention": "20 per p-p, 63 per p-c (FMA = 2, rsqrt = 1)",
@@ -321,6 +323,15 @@ def run_ours(args):
         dist.barrier()
         dist.destroy_process_group()
     return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of k_walk from one `ncu --set full` capture of the default workload
+# (profiles/r1e_walk_ncu.md: 441.7 MB + 262.9 MB per launch); any other configuration has no capture.
+WALK_DRAM_BYTES_NCU = {("plummer_4m", 64, 2, 1024): 704.7e6}
+
+
+def walk_traffic(args):
+    return WALK_DRAM_BYTES_NCU.get((args.workload, args.ncrit, args.group_mode, args.group_cell))
 
 
 def main():
