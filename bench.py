@@ -171,6 +171,26 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------------
+def max_over_ranks(values, world: int, device=None):
+    """The timing rule of the bench contract: every rank's device time, reduced with MAX over the ranks.
+
+    With world == 1 (or no process group) the values come back unchanged.  Works on whatever backend the default
+    process group uses (nccl in the bench, gloo in the CPU test).
+    """
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def aggregate_value(n_per_rank: int, world: int, steps: int, total_ms: float) -> float:
+    """Whole-job throughput of N independent replicas: units all ranks processed / max-over-ranks time."""
+    return world * n_per_rank * steps / (total_ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -263,15 +283,12 @@ def run_ours(args):
     barrier()
     e2e_total_ms = float(sum(e2e_ms))
 
-    if world > 1:
-        t = torch.tensor([total_ms, e2e_total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, e2e_total_ms = float(t[0]), float(t[1])
+    total_ms, e2e_total_ms = max_over_ranks([total_ms, e2e_total_ms], world, dev)
 
     if rank == 0:
         ms_per_step = total_ms / args.steps
-        value = world * n * args.steps / (total_ms * 1e-3)
-        e2e_value = world * n * args.steps / (e2e_total_ms * 1e-3)
+        value = aggregate_value(n, world, args.steps, total_ms)
+        e2e_value = aggregate_value(n, world, args.steps, e2e_total_ms)
         st = {k: float(np.mean([s[k] for s in stage_ms])) for k in stage_ms[0] if k != "integrate"}
         walk_ms = st["walk"]
         flop = FLOP_PP * sum_pp + FLOP_PC * sum_pc
