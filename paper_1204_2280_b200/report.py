@@ -1,0 +1,149 @@
+"""Measurements of the BASELINE.json configurations that are not the bench line (python -m paper_1204_2280_b200.report).
+
+  configs[1]  N = 2^18: theta sweep {0.3, 0.5, 0.75, 1.0}, interactions per particle and walk time
+  configs[2]  N = 2^20: 8 KDK leapfrog steps (dt = 1/1024, shared step, tree rebuilt every step) at theta = 0.5, 0.75
+  configs[4]  N = 2^20: walk of an active subset (N/16, N/256; scattered and clustered) against the full walk,
+              with the tree rebuilt and with the tree refreshed (bonsai_refresh_tree)
+  scaling     N = 2^15 ... 2^22: time per stage (the paper's Fig. 2 quantity)
+
+Everything runs through the C-ABI binding on cuda:0 with seeded synthetic Plummer spheres; times are CUDA-event
+stage times of the library (median of `--reps`), L2 not flushed between repetitions.  Prints one JSON document.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import numpy as np
+import torch
+
+from . import Bonsai
+from . import workloads as W
+
+
+def _median_stage(b: Bonsai, fn, reps: int) -> dict:
+    rows = []
+    for _ in range(reps):
+        fn()
+        rows.append(b.stage_ms())
+    return {k: float(np.median([r[k] for r in rows])) for k in rows[0]}
+
+
+def theta_sweep(reps: int) -> dict:
+    cfg = W.CONFIGS["plummer_256k"]
+    n, eps = cfg["n"], cfg["eps"]
+    pm = torch.from_numpy(W.plummer(n)).cuda()
+    b = Bonsai(n)
+    b.set_timing(True)
+    out = {}
+    for theta in cfg["theta_sweep"]:
+        b.step(pm, theta, eps)
+        b.sync()
+        st = _median_stage(b, lambda: b.step(pm, theta, eps), reps)
+        pp, pc = b.interaction_totals()
+        out[str(theta)] = {"pp_per_particle": pp / n, "pc_per_particle": pc / n, "walk_ms": st["walk"],
+                           "step_ms": sum(v for k, v in st.items() if k != "integrate")}
+    return {"n": n, "eps": eps, "by_theta": out}
+
+
+def leapfrog(reps: int) -> dict:
+    cfg = W.CONFIGS["plummer_1m"]
+    n, eps, dt, steps = cfg["n"], cfg["eps"], 1.0 / 1024, 8
+    pm_h, vel_h = W.plummer(n, with_velocities=True)
+    v4 = np.zeros((n, 4), np.float32)
+    v4[:, :3] = vel_h
+    res = {}
+    for theta in (0.5, 0.75):
+        pm, vel = torch.from_numpy(pm_h).cuda(), torch.from_numpy(v4).cuda()
+        b = Bonsai(n)
+        acc = b.step(pm, theta, eps).clone()
+        d0 = b.diagnostics(pm, vel, acc).cpu().numpy()
+        b.leapfrog_step(pm, vel, acc, theta, eps, dt)            # warm-up step (counts as step 1 of the run)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b.sync()
+        with torch.cuda.stream(b.stream):
+            e0.record()
+        for _ in range(steps - 1):
+            b.leapfrog_step(pm, vel, acc, theta, eps, dt)
+        with torch.cuda.stream(b.stream):
+            e1.record()
+        b.sync()
+        d1 = b.diagnostics(pm, vel, acc).cpu().numpy()
+        ms = e0.elapsed_time(e1) / (steps - 1)
+        res[str(theta)] = {"ms_per_step": ms, "particle_steps_per_s": n / (ms * 1e-3),
+                           "rel_energy_drift_8_steps": float(abs((d1[0] + d1[1]) / (d0[0] + d0[1]) - 1.0))}
+    return {"n": n, "eps": eps, "dt": dt, "steps": steps, "by_theta": res}
+
+
+def block_step(reps: int) -> dict:
+    cfg = W.CONFIGS["plummer_1m"]
+    n, eps, theta = cfg["n"], cfg["eps"], cfg["theta"]
+    pm_h, vel_h = W.plummer(n, with_velocities=True)
+    v4 = np.zeros((n, 4), np.float32)
+    v4[:, :3] = vel_h
+    pm, vel = torch.from_numpy(pm_h).cuda(), torch.from_numpy(v4).cuda()
+    b = Bonsai(n)
+    b.set_timing(True)
+    out = b.step(pm, theta, eps)
+    b.sync()
+    full = _median_stage(b, lambda: b.step(pm, theta, eps, out=out), reps)
+    pre = sum(v for k, v in full.items() if k not in ("walk", "integrate"))
+    res = {"n": n, "theta": theta, "full_walk_ms": full["walk"], "full_pre_walk_ms": pre, "subsets": {}}
+    for pattern in ("clustered", "scattered"):
+        for frac in (16, 256):
+            mask = torch.from_numpy(W.active_mask(pm_h, n // frac, pattern)).cuda()
+            st = _median_stage(b, lambda: b.step(pm, theta, eps, mask, out=out), reps)
+            res["subsets"][f"{pattern}_N/{frac}"] = {
+                "walk_ms": st["walk"], "groups_ms": st["groups"], "walk_time_reduction": full["walk"] / st["walk"],
+                "ideal": frac}
+    # refreshed tree instead of a rebuild: drift a little, refresh, recompute multipoles, walk the clustered N/16 subset
+    mask = torch.from_numpy(W.active_mask(pm_h, n // 16, "clustered")).cuda()
+
+    def refreshed():
+        b.drift(pm, vel, 1.0 / 1024)
+        b.refresh_tree()
+        b.compute_multipoles()
+        b.walk(theta, eps, mask, out=out)
+
+    st = _median_stage(b, refreshed, reps)
+    res["refreshed_clustered_N/16"] = {"reorder_ms": st["reorder"], "groups_ms": st["groups"],
+                                       "multipoles_ms": st["multipoles"], "walk_ms": st["walk"],
+                                       "step_ms": st["reorder"] + st["groups"] + st["multipoles"] + st["walk"],
+                                       "rebuild_step_ms": pre + res["subsets"]["clustered_N/16"]["walk_ms"]}
+    return res
+
+
+def scaling(reps: int) -> dict:
+    rows = {}
+    for name in ("plummer_32k", "plummer_256k", "plummer_1m", "plummer_4m"):
+        cfg = W.CONFIGS[name]
+        n, eps, theta = cfg["n"], cfg["eps"], cfg["theta"]
+        pm = torch.from_numpy(W.plummer(n)).cuda()
+        b = Bonsai(n)
+        b.set_timing(True)
+        b.step(pm, theta, eps)
+        b.sync()
+        st = _median_stage(b, lambda: b.step(pm, theta, eps), reps)
+        pp, pc = b.interaction_totals()
+        st.pop("integrate", None)
+        total = sum(st.values())
+        rows[name] = {"n": n, "stage_ms": st, "step_ms": total, "particles_per_s": n / (total * 1e-3),
+                      "walk_share": st["walk"] / total, "pp_per_particle": pp / n, "pc_per_particle": pc / n}
+        del b
+    return rows
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling"), default=None)
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("report: no CUDA device -- libbonsai has no CPU fallback")
+    parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "scaling": scaling}
+    doc = {k: f(args.reps) for k, f in parts.items() if args.only in (None, k)}
+    print(json.dumps(doc, indent=1))
+
+
+if __name__ == "__main__":
+    main()
