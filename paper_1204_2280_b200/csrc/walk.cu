@@ -14,7 +14,7 @@
 //   rejected internal  -> its child run is pushed.
 // Few groups (a small active subset): one group's walk is a serial chain of ~0.4 ms, so when there are fewer
 // groups than resident warps the kernel would last as long as its slowest group.  The warps of a block then form
-// TEAMS of S = 2, 4 or 8 (the largest S with n_groups * S <= resident warps): every warp of a team runs the same
+// TEAMS of S = 2, 4 or 8 (chosen on the device from the number of groups): every warp of a team runs the same
 // traversal of the same group (same opening tests, same lists, same counts) but evaluates only every S-th batch of
 // 32 interactions, and the team's partial sums are folded in a fixed order at the end.  The traversal is ~15 % of a
 // group's time, so a team of 8 finishes a group ~4x sooner.
@@ -499,10 +499,18 @@ __global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
     WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[w];
     const uint32_t n_groups = a.ctl->n_groups;
     if constexpr (kTeams) {
-        // team size: the largest power of two <= warps per block that still leaves every resident warp a group
+        // team size S in {1, 2, 4, 8}: with dynamic tickets the kernel lasts about ceil(n_groups S / warps) rounds of
+        // one group-walk each, and a team of S shortens a group-walk to ~(0.15 + 0.85 / S) of a single warp's (the
+        // traversal, ~15 %, is repeated by every member; measured, profiles/r1f_configs.md).  Take the cheapest S,
+        // the smaller one on near-ties.
         const uint32_t warps = gridDim.x * kWalkWarps;
         int tsize = 1;
-        while (tsize < kWalkWarps && (unsigned long long)n_groups * (2 * tsize) <= warps) tsize *= 2;
+        float best = 3.0e38f;
+        for (int S = 1; S <= kWalkWarps; S *= 2) {
+            const float rounds = (float)(((unsigned long long)n_groups * S + warps - 1) / warps);
+            const float cost = rounds * (0.15f + 0.85f / (float)S);
+            if (cost < 0.95f * best) { best = cost; tsize = S; }
+        }
         if (tsize > 1) {
             walk_groups<kZeroEps, true>(S, a, n_groups, lane, w, tsize, s_team_g);
             return;
