@@ -61,17 +61,19 @@ __global__ void __launch_bounds__(256) k_groups_mark(const Control* __restrict__
                                                      const uint32_t* __restrict__ c_parent,
                                                      const uint32_t* __restrict__ rank, uint32_t* __restrict__ g_flag,
                                                      uint32_t* __restrict__ g_cell) {
-    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= min(ctl->n_cells, cap_cells)) return;
-    const uint32_t cnt = c_count[c];
-    if (!(cnt <= limit || c_n_child[c] == 0)) return;
-    const uint32_t p = c_parent[c];
-    if (p != kNone && c_count[p] <= limit) return;  // an ancestor already is the group / container
-    const uint32_t f = c_first[c];
-    const uint32_t a = rank[f + cnt] - rank[f];
-    if (a == 0) return;                              // no active member
-    g_flag[f] = chunk ? (a + chunk - 1u) / chunk : 1u;  // number of groups this cell contributes
-    g_cell[f] = c + 1u;
+    // grid-stride: the number of cells is only known on the device
+    const uint32_t n_cells = min(ctl->n_cells, cap_cells);
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += gridDim.x * blockDim.x) {
+        const uint32_t cnt = c_count[c];
+        if (!(cnt <= limit || c_n_child[c] == 0)) continue;
+        const uint32_t p = c_parent[c];
+        if (p != kNone && c_count[p] <= limit) continue;  // an ancestor already is the group / container
+        const uint32_t f = c_first[c];
+        const uint32_t a = rank[f + cnt] - rank[f];
+        if (a == 0) continue;                              // no active member
+        g_flag[f] = chunk ? (a + chunk - 1u) / chunk : 1u;  // number of groups this cell contributes
+        g_cell[f] = c + 1u;
+    }
 }
 
 // mode 0, step 2 (after the scan of g_flag): first / count of every group
@@ -157,7 +159,7 @@ cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order) {
         const bool cells = (c->prm.group_mode == 0);
         const uint32_t limit = cells ? c->prm.ncrit : c->prm.group_cell;
         const uint32_t chunk = cells ? 0u : c->prm.ncrit;
-        k_groups_mark<<<div_up(c->cap_cells, 256), 256, 0, c->stream>>>(b.ctl, c->cap_cells, limit, chunk, b.c_first,
+        k_groups_mark<<<min(div_up(c->cap_cells, 256), (uint32_t)c->num_sms * 16u), 256, 0, c->stream>>>(b.ctl, c->cap_cells, limit, chunk, b.c_first,
                                                                         b.c_count, b.c_n_child, b.c_parent, b.rank,
                                                                         b.g_flag, b.g_cell);
         c->launches += 1;

@@ -246,11 +246,13 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_emit(const int8_t* __rest
 
 __global__ void __launch_bounds__(256) k_tree_finalize(const Control* __restrict__ ctl, uint32_t cap_cells,
                                                        CellArrays ca) {
-    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= min(ctl->n_cells, cap_cells)) return;
-    ca.count[c] = ca.count[c] - ca.first[c];
-    const uint32_t fc = ca.first_child[c];
-    if (fc != 0) ca.n_child[c] = ca.n_child[c] - fc + 1u;
+    // grid-stride: the number of cells is only known on the device, a grid sized for cap_cells would be mostly empty
+    const uint32_t n_cells = min(ctl->n_cells, cap_cells);
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += gridDim.x * blockDim.x) {
+        ca.count[c] = ca.count[c] - ca.first[c];
+        const uint32_t fc = ca.first_child[c];
+        if (fc != 0) ca.n_child[c] = ca.n_child[c] - fc + 1u;
+    }
 }
 
 cudaError_t stage_build(Ctx* c) {
@@ -266,7 +268,7 @@ cudaError_t stage_build(Ctx* c) {
                                                              c->cap_cells);
     k_tree_emit<<<n_blocks, kTreeThreads, 0, c->stream>>>(b.lcp, b.leaf_level, n, n_blocks, b.blk_level_count, b.ctl,
                                                           c->cap_cells, ca);
-    k_tree_finalize<<<div_up(c->cap_cells, 256), 256, 0, c->stream>>>(b.ctl, c->cap_cells, ca);
+    k_tree_finalize<<<min(div_up(c->cap_cells, 256), (uint32_t)c->num_sms * 16u), 256, 0, c->stream>>>(b.ctl, c->cap_cells, ca);
     c->launches += 5;
     return cudaGetLastError();
 }
