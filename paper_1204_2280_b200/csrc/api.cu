@@ -204,7 +204,11 @@ int bonsai_build_tree(bonsai_ctx* h) {
     { StageTimer t(c, 0); BONSAI_TRY(stage_bbox(c)); }
     { StageTimer t(c, 1); BONSAI_TRY(stage_keys(c)); }
     { StageTimer t(c, 2); BONSAI_TRY(stage_sort(c)); }
-    { StageTimer t(c, 3); BONSAI_TRY(stage_reorder(c, true)); }
+    {
+        StageTimer t(c, 3);
+        BONSAI_TRY(stage_reorder(c, true));
+        BONSAI_TRY(stage_sort_ties(c));
+    }
     { StageTimer t(c, 4); BONSAI_TRY(stage_build(c)); }
     { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
     c->tree_n = c->n;

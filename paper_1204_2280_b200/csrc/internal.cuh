@@ -54,7 +54,8 @@ struct Control {
     uint32_t level_ticket;     // last-block-done counter of k_tree_scan_levels
     uint32_t sort_ticket;      // tile scheduler of k_sort_pass (reset by the tile that draws the last ticket)
     uint32_t diag_ticket;      // last-block-done counter of k_diagnostics
-    uint32_t pad1[4];
+    uint32_t sort_fallback;    // set by k_sort_ties when a run of equal (hi, mid) is too long: the guarded chain runs
+    uint32_t pad1[3];
     uint32_t level_offsets[32];  // first cell of level L; [31] = n_cells
     unsigned long long sum_pp;   // interaction totals of the last walk (sink-source pairs)
     unsigned long long sum_pc;
@@ -147,6 +148,7 @@ cudaError_t stage_bbox(Ctx* c);
 cudaError_t stage_keys(Ctx* c);
 cudaError_t stage_sort(Ctx* c);
 cudaError_t stage_reorder(Ctx* c, bool write_keys);
+cudaError_t stage_sort_ties(Ctx* c);
 cudaError_t stage_build(Ctx* c);
 cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order);
 cudaError_t stage_multipoles(Ctx* c);

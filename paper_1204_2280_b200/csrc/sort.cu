@@ -155,8 +155,9 @@ __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict_
 }
 
 // exclusive scan of each pass's histogram: ghist[p][d] <- sum_{d' < d} ghist[p][d'].  One block per pass.
-__global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ ghist) {
+__global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ ghist, Control* __restrict__ ctl) {
     __shared__ uint32_t wsum[kRadix / 32];
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->sort_fallback = 0;
     uint32_t* h = ghist + blockIdx.x * kRadix;
     uint32_t v = h[threadIdx.x];
     uint32_t x = v;
@@ -211,6 +212,7 @@ struct SortPass {
     const uint32_t* gbase;     // [kRadix] exclusive digit bases of this pass
     unsigned long long* look;  // [n_tiles][kRadix]
     uint32_t* ticket;
+    const uint32_t* guard;     // nullptr, or a device flag: the pass only runs when it is non-zero (fallback chain)
     uint32_t n, n_tiles, epoch;
     int shift;
 };
@@ -243,6 +245,7 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
     __shared__ uint32_t s_tile;
     __shared__ uint32_t s_wsum[kWarps];
     const int tid = threadIdx.x, l = tid & 31, w = tid >> 5;
+    if (a.guard != nullptr && __ldg(a.guard) == 0u) return;  // uniform over the grid: the flag was set before the launch
 
     if (tid == 0) {
         const uint32_t t = atomicAdd(a.ticket, 1u);
@@ -432,17 +435,20 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
 __global__ void __launch_bounds__(256) k_reorder(const float4* __restrict__ pos, const uint32_t* __restrict__ perm,
                                                  uint32_t n, const Control* __restrict__ ctl,
                                                  float4* __restrict__ sorted_pos, uint32_t* __restrict__ khi,
-                                                 uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo) {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const float4 p = __ldg(&pos[__ldg(&perm[i])]);
-    sorted_pos[i] = p;
-    if (khi == nullptr) return;  // refresh of a frozen tree (R25): the keys stay those of the last build
-    uint32_t w[3];
-    morton_words(p, ctl->lo[0], ctl->lo[1], ctl->lo[2], ctl->scale, w);
-    klo[i] = w[0];
-    kmid[i] = w[1];
-    khi[i] = w[2];
+                                                 uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
+                                                 const uint32_t* __restrict__ guard) {
+    if (guard != nullptr && __ldg(guard) == 0u) return;
+    const float lox = ctl->lo[0], loy = ctl->lo[1], loz = ctl->lo[2], scale = ctl->scale;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float4 p = __ldg(&pos[__ldg(&perm[i])]);
+        sorted_pos[i] = p;
+        if (khi == nullptr) continue;  // refresh of a frozen tree (R25): the keys stay those of the last build
+        uint32_t w[3];
+        morton_words(p, lox, loy, loz, scale, w);
+        klo[i] = w[0];
+        kmid[i] = w[1];
+        khi[i] = w[2];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -464,11 +470,75 @@ cudaError_t stage_keys(Ctx* c) {
     return cudaGetLastError();
 }
 
-cudaError_t stage_sort(Ctx* c) {
-    const uint32_t n = c->n;
-    Buffers& b = c->b;
+// Ties of the two-word sort.  After the six passes over the mid and hi words the particles are ordered by their
+// first 20 octal digits and, inside a run of equal digits, by load index (LSD passes are stable).  Such runs are
+// cells of side 2^-20 of the root cube: with fp32 coordinates they hold one particle almost always.  The thread
+// at the head of a run orders it by (lo word, load index) with an insertion sort over perm, sorted_pos and the lo
+// keys; a run longer than kTieRun raises the fallback flag instead and the guarded nine-pass chain redoes the sort.
+constexpr uint32_t kTieRun = 32;
+
+__device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, const uint32_t* __restrict__ khi,
+                                          const uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
+                                          uint32_t* __restrict__ perm, float4* __restrict__ sorted_pos, uint32_t n,
+                                          Control* __restrict__ ctl) {
+    uint32_t len = 2;
+    while (i + len < n && len <= kTieRun && khi[i + len] == h && kmid[i + len] == m) ++len;
+    if (len > kTieRun) {
+        ctl->sort_fallback = 1;
+        return;
+    }
+    for (uint32_t k = 1; k < len; ++k) {  // stable insertion sort by lo: equal lo keep their ascending load index
+        const uint32_t lo = klo[i + k], pk = perm[i + k];
+        const float4 xk = sorted_pos[i + k];
+        uint32_t j = k;
+        while (j > 0 && klo[i + j - 1] > lo) {
+            klo[i + j] = klo[i + j - 1];
+            perm[i + j] = perm[i + j - 1];
+            sorted_pos[i + j] = sorted_pos[i + j - 1];
+            --j;
+        }
+        klo[i + j] = lo;
+        perm[i + j] = pk;
+        sorted_pos[i + j] = xk;
+    }
+}
+
+// Four consecutive sorted particles per thread (16-byte loads of the hi and mid words plus one neighbour on each
+// side); a particle that ties with its successor but not with its predecessor heads a run.
+__global__ void __launch_bounds__(256) k_sort_ties(const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
+                                                   uint32_t* __restrict__ klo, uint32_t* __restrict__ perm,
+                                                   float4* __restrict__ sorted_pos, uint32_t n, Control* __restrict__ ctl) {
+    const uint32_t i0 = 4u * (blockIdx.x * blockDim.x + threadIdx.x);
+    if (i0 >= n) return;
+    uint32_t h[6], m[6];  // positions i0 - 1 .. i0 + 4; out-of-range slots get a value no key has
+    if (i0 + 4 <= n) {
+        const uint4 hv = __ldg(reinterpret_cast<const uint4*>(khi + i0)), mv = __ldg(reinterpret_cast<const uint4*>(kmid + i0));
+        h[1] = hv.x; h[2] = hv.y; h[3] = hv.z; h[4] = hv.w;
+        m[1] = mv.x; m[2] = mv.y; m[3] = mv.z; m[4] = mv.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            h[1 + k] = (i0 + k < n) ? __ldg(&khi[i0 + k]) : 0xFFFFFFFFu;
+            m[1 + k] = (i0 + k < n) ? __ldg(&kmid[i0 + k]) : 0xFFFFFFFFu;
+        }
+    }
+    h[0] = (i0 > 0) ? __ldg(&khi[i0 - 1]) : 0xFFFFFFFFu;
+    m[0] = (i0 > 0) ? __ldg(&kmid[i0 - 1]) : 0xFFFFFFFFu;
+    h[5] = (i0 + 4 < n) ? __ldg(&khi[i0 + 4]) : 0xFFFFFFFFu;
+    m[5] = (i0 + 4 < n) ? __ldg(&kmid[i0 + 4]) : 0xFFFFFFFFu;
+#pragma unroll
+    for (int k = 1; k <= 4; ++k) {
+        if (h[k] == 0xFFFFFFFFu) break;  // past the end (key words have 30 bits)
+        const bool ties_next = (h[k + 1] == h[k]) && (m[k + 1] == m[k]);
+        const bool ties_prev = (h[k - 1] == h[k]) && (m[k - 1] == m[k]);
+        if (ties_next && !ties_prev) sort_tie_run(i0 + k - 1, h[k], m[k], khi, kmid, klo, perm, sorted_pos, n, ctl);
+    }
+}
+
+static cudaError_t sort_prepare(Ctx* c, size_t* smem_out) {
     static bool attr_set = false;
     const size_t smem = sizeof(uint32_t) * ((kSortThreads / 32) * kRadix + 2 * kRadix);
+    *smem_out = smem;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(k_sort_pass<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_pass<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -476,18 +546,28 @@ cudaError_t stage_sort(Ctx* c) {
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist);
-    c->launches += 1;
+    (void)c;
+    return cudaSuccess;
+}
+
+// Passes first_pass .. 8 of the LSD sort (pass p: word 2 - p / 3 = lo, mid, hi; digit p % 3), starting from the
+// identity permutation.  The first pass writes pair buffer first_out, every later pass flips; with first_out chosen
+// by the callers below both chains leave the permutation in idx[0].
+static cudaError_t sort_chain(Ctx* c, int first_pass, int first_out, const uint32_t* guard) {
+    Buffers& b = c->b;
+    size_t smem;
+    cudaError_t e = sort_prepare(c, &smem);
+    if (e != cudaSuccess) return e;
     SortPass a;
-    a.n = n;
-    a.n_tiles = div_up(n, kSortTile);
+    a.n = c->n;
+    a.n_tiles = div_up(c->n, kSortTile);
     a.look = b.look;
     a.ticket = &b.ctl->sort_ticket;
-    int cur = 0;  // pass p reads pair buffer cur (p > 0) and writes cur ^ 1; pass 0 writes buffer 0
-    for (int p = 0; p < kSortPasses; ++p) {
+    a.guard = guard;
+    int cur = first_out ^ 1;
+    for (int p = first_pass; p < kSortPasses; ++p) {
         if (c->sort_epoch >= (1u << 30) - 1) {  // 30-bit epoch about to wrap: forget every stale entry
-            cudaError_t e = cudaMemsetAsync(b.look, 0, sizeof(unsigned long long) * (size_t)div_up(c->n_max, kSortTile) * kRadix,
-                                            c->stream);
+            e = cudaMemsetAsync(b.look, 0, sizeof(unsigned long long) * (size_t)div_up(c->n_max, kSortTile) * kRadix, c->stream);
             if (e != cudaSuccess) return e;
             c->sort_epoch = 0;
         }
@@ -495,27 +575,56 @@ cudaError_t stage_sort(Ctx* c) {
         a.shift = kRadixBits * (p % 3);
         a.gbase = b.ghist + p * kRadix;
         a.src_word = b.key[0][2 - p / 3];  // load-order word of this phase: lo, mid, hi
-        const int out = (p == 0) ? 0 : (cur ^ 1);
+        const int out = cur ^ 1;
         a.key_in = b.pair_key[cur];
         a.idx_in = b.idx[cur];
         a.key_out = (p == kSortPasses - 1) ? nullptr : b.pair_key[out];
         a.idx_out = b.idx[out];
-        if (p == 0) k_sort_pass<0><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
+        if (p == first_pass) k_sort_pass<0><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
         else if (p % 3 == 0) k_sort_pass<2><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
         else k_sort_pass<1><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
         c->launches += 1;
         cur = out;
     }
-    c->perm = b.idx[cur];
-    return cudaGetLastError();
+    return (cur == 0) ? cudaGetLastError() : cudaErrorUnknown;
+}
+
+// The sort proper: six passes over the mid and hi words (the lo word almost never decides the order, see k_sort_ties).
+cudaError_t stage_sort(Ctx* c) {
+    Buffers& b = c->b;
+    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist, b.ctl);
+    c->launches += 1;
+    c->perm = b.idx[0];
+    return sort_chain(c, 3, 1, nullptr);  // outputs 1, 0, 1, 0, 1, 0
+}
+
+static void launch_reorder(Ctx* c, bool write_keys, const uint32_t* guard) {
+    Buffers& b = c->b;
+    // the guarded instance normally returns at once: keep its grid small
+    const uint32_t blocks = guard ? (uint32_t)c->num_sms * 8u : div_up(c->n, 256);
+    k_reorder<<<blocks, 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos,
+                                             write_keys ? b.key[1][0] : nullptr, b.key[1][1], b.key[1][2], guard);
+    c->launches += 1;
 }
 
 cudaError_t stage_reorder(Ctx* c, bool write_keys) {
-    Buffers& b = c->b;
-    k_reorder<<<div_up(c->n, 256), 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos,
-                                                        write_keys ? b.key[1][0] : nullptr, b.key[1][1], b.key[1][2]);
+    launch_reorder(c, write_keys, nullptr);
     c->sorted_buf = 1;
+    return cudaGetLastError();
+}
+
+// After the reorder of a fresh sort: order the (rare) runs of equal (hi, mid) by their lo word, and keep the full
+// nine-pass chain plus a second reorder enqueued behind the fallback flag for inputs with long runs (coincident
+// particles, clusters far smaller than 2^-20 of the box).  The guarded launches return at once in the normal case.
+cudaError_t stage_sort_ties(Ctx* c) {
+    Buffers& b = c->b;
+    k_sort_ties<<<div_up(div_up(c->n, 4), 256), 256, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
+                                                          b.ctl);
     c->launches += 1;
+    const uint32_t* guard = &b.ctl->sort_fallback;
+    cudaError_t e = sort_chain(c, 0, 0, guard);  // outputs 0, 1, 0, 1, 0, 1, 0, 1, 0
+    if (e != cudaSuccess) return e;
+    launch_reorder(c, true, guard);
     return cudaGetLastError();
 }
 

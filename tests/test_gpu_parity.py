@@ -228,6 +228,34 @@ def test_duplicate_positions_and_deep_chain():
     check_walk(b, out, ref, count_frac=0.98, eps=0.01, pm=pm)
 
 
+@pytest.mark.parametrize("clump_sizes", [(2, 3, 5, 17, 32), (33, 40, 200), (2, 31, 32, 33)])
+def test_sort_ties_below_the_20th_level(clump_sizes):
+    """The sort orders by the mid and hi key words and repairs runs of equal (hi, mid) afterwards (sort.cu): clumps
+    far smaller than 2^-20 of the root cube with DISTINCT positions inside exercise the in-place repair (runs
+    <= 32) and the guarded nine-pass fallback (longer runs).  The permutation must still be the oracle's."""
+    rng = np.random.default_rng(sum(clump_sizes))
+    n = 6000
+    pm = W.plummer(n)
+    pm[0, :3] = (900.0, -700.0, 800.0)                       # a far particle: root cube side 2048, 2^-20 side = 2e-3
+    at = 100
+    for k, sz in enumerate(clump_sizes):
+        centre = pm[at, :3].copy()
+        # distinct fp32 positions within ~1e-5 of the centre: same first 20 digits, different lo words
+        off = (rng.integers(-40, 41, size=(sz, 3)) * np.float32(2.0 ** -22)).astype(np.float32)
+        pm[at:at + sz, :3] = centre + off
+        at += sz + 50
+    pm = pm[rng.permutation(n)]
+    ref = O.full_step(pm, 0.75, 0.01)
+    # the scenario is what it claims to be: runs of equal (hi, mid) with several lo values inside
+    k = ref.sorted_keys
+    tie = (k[1:, 0] == k[:-1, 0]) & (k[1:, 1] == k[:-1, 1])
+    assert tie.sum() >= sum(clump_sizes) - len(clump_sizes) - 2 and (k[1:, 2][tie] != k[:-1, 2][tie]).any()
+    b, out = run_gpu(pm, 0.75, 0.01)
+    check_structure(b, ref)
+    check_groups(b, ref)
+    check_walk(b, out, ref, count_frac=0.98, eps=0.01, pm=pm)
+
+
 def test_all_particles_coincident():
     pm = np.zeros((100, 4), np.float32)
     pm[:, :3] = (1.0, 2.0, 3.0)
