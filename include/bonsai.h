@@ -146,7 +146,8 @@ typedef struct {
                                       then u32 link (leaf: first particle; else first child) and u32 info
                                       (leaf: 0x80000000 | count; else n_child)                                */
     const float* quad;             /* device, 6 floats per cell: xx, yy, zz, xy, xz, yz (raw second moments
-                                      about the COM, R8)                                                     */
+                                      about the COM, R8); filled by bonsai_get_cells() itself (one small
+                                      kernel on the stream), valid after bonsai_compute_multipoles()        */
     const float* walk_quad;        /* device, 8 floats per cell, the walk's second record: P = tr I - 3 Q as
                                       Pxx, Pyy, Pzz, Pxy, Pxz, Pyz, then tr = Qxx + Qyy + Qzz and a pad      */
 } bonsai_cells_view;

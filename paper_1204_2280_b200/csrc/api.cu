@@ -393,6 +393,7 @@ int bonsai_get_cells(bonsai_ctx* h, bonsai_cells_view* out) {
     if (!h || !out) return BONSAI_EINVAL;
     if (h->c.state < 2) return BONSAI_ESTATE;
     const Buffers& b = h->c.b;
+    if (h->c.state >= 3) BONSAI_TRY(cells_qraw(&h->c));  // quad[] is derived from the fp64 record on demand
     out->cap_cells = h->c.cap_cells;
     out->n_cells = &b.ctl->n_cells;
     out->level_offsets = b.ctl->level_offsets;

@@ -152,6 +152,7 @@ cudaError_t stage_sort_ties(Ctx* c);
 cudaError_t stage_build(Ctx* c);
 cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order);
 cudaError_t stage_multipoles(Ctx* c);
+cudaError_t cells_qraw(Ctx* c);  // fills c_qraw from c_mom (introspection)
 cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out);
 size_t walk_smem_bytes(uint32_t nleaf);
 cudaError_t stage_kick(Ctx* c, float4* vel, const float4* acc, uint32_t n, float h, const uint8_t* mask);

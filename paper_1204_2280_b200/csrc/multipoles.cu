@@ -66,10 +66,13 @@ __device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], c
     }
     const double ex = __dadd_rn(o.cx, -g[0]), ey = __dadd_rn(o.cy, -g[1]), ez = __dadd_rn(o.cz, -g[2]);
     const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
-    double* mo = c_mom + (size_t)c * 10;
-    __stcg(&mo[0], o.m); __stcg(&mo[1], o.cx); __stcg(&mo[2], o.cy); __stcg(&mo[3], o.cz);
-    __stcg(&mo[4], o.xx); __stcg(&mo[5], o.yy); __stcg(&mo[6], o.zz);
-    __stcg(&mo[7], o.xy); __stcg(&mo[8], o.xz); __stcg(&mo[9], o.yz);
+    // 16-byte stores: the record is written (and read back by the parent) in 5 L2 transactions instead of 10
+    double2* mo = reinterpret_cast<double2*>(c_mom + (size_t)c * 10);
+    __stcg(&mo[0], make_double2(o.m, o.cx));
+    __stcg(&mo[1], make_double2(o.cy, o.cz));
+    __stcg(&mo[2], make_double2(o.xx, o.yy));
+    __stcg(&mo[3], make_double2(o.zz, o.xy));
+    __stcg(&mo[4], make_double2(o.xz, o.yz));
     CellMac cm;
     cm.cx = (float)o.cx; cm.cy = (float)o.cy; cm.cz = (float)o.cz; cm.m = (float)o.m;
     cm.delta = (float)sqrt(d2);
@@ -77,9 +80,7 @@ __device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], c
     cm.first = link_first;
     cm.info = link_info;
     c_mac[c] = cm;
-    float* qr = c_qraw + (size_t)c * 6;
-    qr[0] = (float)o.xx; qr[1] = (float)o.yy; qr[2] = (float)o.zz;
-    qr[3] = (float)o.xy; qr[4] = (float)o.xz; qr[5] = (float)o.yz;
+    (void)c_qraw;  // the fp32 raw moments are introspection only: k_cells_qraw derives them from c_mom on demand
     const double tr = o.xx + o.yy + o.zz;
     CellQuad cq;
     cq.pxx = (float)(tr - 3.0 * o.xx); cq.pyy = (float)(tr - 3.0 * o.yy); cq.pzz = (float)(tr - 3.0 * o.zz);
@@ -157,34 +158,37 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
         q.m = 0.0;
         for (uint32_t k = 0; k < nc; ++k) {
-            const double* mo = c_mom + (size_t)(fc + k) * 10;
+            const double2* mo = reinterpret_cast<const double2*>(c_mom + (size_t)(fc + k) * 10);
             if (use_extent) {
                 const float2* bx = reinterpret_cast<const float2*>(c_box + (size_t)(fc + k) * 6);
                 const float2 b0 = __ldcg(&bx[0]), b1 = __ldcg(&bx[1]), b2 = __ldcg(&bx[2]);
                 mn[0] = fminf(mn[0], b0.x); mn[1] = fminf(mn[1], b0.y); mn[2] = fminf(mn[2], b1.x);
                 mx[0] = fmaxf(mx[0], b1.y); mx[1] = fmaxf(mx[1], b2.x); mx[2] = fmaxf(mx[2], b2.y);
             }
-            const double m = __ldcg(&mo[0]);
+            const double2 r0 = __ldcg(&mo[0]), r1 = __ldcg(&mo[1]);  // (m, cx), (cy, cz)
+            const double m = r0.x;
             q.m += m;
-            sx += m * __ldcg(&mo[1]);
-            sy += m * __ldcg(&mo[2]);
-            sz += m * __ldcg(&mo[3]);
+            sx += m * r0.y;
+            sy += m * r1.x;
+            sz += m * r1.y;
         }
         q.cx = q.cy = q.cz = 0.0;
         q.xx = q.yy = q.zz = q.xy = q.xz = q.yz = 0.0;
         if (q.m > 0.0) {
             q.cx = sx / q.m; q.cy = sy / q.m; q.cz = sz / q.m;
             for (uint32_t k = 0; k < nc; ++k) {
-                const double* mo = c_mom + (size_t)(fc + k) * 10;
-                const double m = __ldcg(&mo[0]);
+                const double2* mo = reinterpret_cast<const double2*>(c_mom + (size_t)(fc + k) * 10);
+                const double2 r0 = __ldcg(&mo[0]), r1 = __ldcg(&mo[1]), r2 = __ldcg(&mo[2]), r3 = __ldcg(&mo[3]),
+                              r4 = __ldcg(&mo[4]);
+                const double m = r0.x;
                 if (!(m > 0.0)) continue;  // a massless child carries the geometric centre, not a COM
-                const double dx = __ldcg(&mo[1]) - q.cx, dy = __ldcg(&mo[2]) - q.cy, dz = __ldcg(&mo[3]) - q.cz;
-                q.xx += __ldcg(&mo[4]) + m * dx * dx;
-                q.yy += __ldcg(&mo[5]) + m * dy * dy;
-                q.zz += __ldcg(&mo[6]) + m * dz * dz;
-                q.xy += __ldcg(&mo[7]) + m * dx * dy;
-                q.xz += __ldcg(&mo[8]) + m * dx * dz;
-                q.yz += __ldcg(&mo[9]) + m * dy * dz;
+                const double dx = r0.y - q.cx, dy = r1.x - q.cy, dz = r1.y - q.cz;
+                q.xx += r2.x + m * dx * dx;
+                q.yy += r2.y + m * dy * dy;
+                q.zz += r3.x + m * dz * dz;
+                q.xy += r3.y + m * dx * dy;
+                q.xz += r4.x + m * dx * dz;
+                q.yz += r4.y + m * dy * dz;
             }
         }
         const uint32_t f = t.first[p];
@@ -192,6 +196,21 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
                    c_mom, c_box, c_mac, c_quad, c_qraw);
         c = p;
     }
+}
+
+// Introspection (bonsai_get_cells): the six raw second moments as fp32, rounded once from the fp64 record (R8).
+__global__ void __launch_bounds__(256) k_cells_qraw(const Control* __restrict__ ctl, uint32_t cap_cells,
+                                                    const double* __restrict__ c_mom, float* __restrict__ c_qraw) {
+    const uint32_t n_cells = min(ctl->n_cells, cap_cells);
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += gridDim.x * blockDim.x)
+#pragma unroll
+        for (int k = 0; k < 6; ++k) c_qraw[(size_t)c * 6 + k] = (float)c_mom[(size_t)c * 10 + 4 + k];
+}
+
+cudaError_t cells_qraw(Ctx* c) {
+    k_cells_qraw<<<c->num_sms * 8, 256, 0, c->stream>>>(c->b.ctl, c->cap_cells, c->b.c_mom, c->b.c_qraw);
+    c->launches += 1;
+    return cudaGetLastError();
 }
 
 cudaError_t stage_multipoles(Ctx* c) {
