@@ -299,9 +299,10 @@ def run_ours(args):
         hbm = peaks.get("hbm_gbs", 6650.0)
         hbm_src = "measured" if "hbm_gbs" in peaks else "fallback"
         # algorithmic bytes per particle of the HBM-bound stages
-        # keys: 16 in + 3 words out; sort: 9 pair passes x (8 in + 8 out), minus the index read of pass 0 (iota) and
-        # the key write of pass 8; reorder: perm + record in, record + 3 key words out
-        alg_bytes = {"bbox": 16, "keys": 28, "sort": 9 * 16 - 8, "reorder": 48, "groups": 16 + 24 / args.ncrit}
+        # keys: 16 in + 3 words out; sort: 6 pair passes over the mid and hi words x (8 in + 8 out), minus the index
+        # read of the first pass (iota) and the key write of the last; reorder: perm + record in, record + 3 key
+        # words out, plus the tie check re-reading the hi and mid words
+        alg_bytes = {"bbox": 16, "keys": 28, "sort": 6 * 16 - 8, "reorder": 48 + 8, "groups": 16 + 24 / args.ncrit}
         stages = {}
         for k, v in st.items():
             ent = {"ms": v, "share": v / sum(st.values())}
