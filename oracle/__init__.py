@@ -343,3 +343,56 @@ def refreshed_step(prev: Step, pos_mass, theta, eps, sel=None, **kw) -> Step:
     s = refresh(prev, pos_mass, **kw)
     s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
     return s
+
+
+# ---- block time-steps (oracle/integrator_oracle.cpp, R26-R27) ------------------------------
+
+def rungs(acc_pot, eta, eps, dt_max, kmax, rung=None, mask=None, tick=0):
+    """rung is None: fresh assignment (R26) -> uint8[n].  Otherwise the R27 update of `rung` in place at `tick`."""
+    ap = _f32(acc_pot)
+    n = ap.shape[0]
+    init = rung is None
+    if init:
+        rung = np.zeros(n, np.uint8)
+    assert rung.dtype == np.uint8 and rung.flags.c_contiguous
+    m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+    lib().oracle_rungs(_p(ap, C.c_float), C.c_uint32(n), C.c_float(eta), C.c_float(eps), C.c_float(dt_max),
+                       C.c_uint32(kmax), _p(m, C.c_uint8), C.c_uint64(tick), _p(rung, C.c_uint8), C.c_int(int(init)))
+    return rung
+
+
+def active_at(rung, kmax, tick):
+    r = np.ascontiguousarray(rung, np.uint8)
+    mask = np.zeros(r.shape[0], np.uint8)
+    lib().oracle_active_mask(_p(r, C.c_uint8), C.c_uint32(r.shape[0]), C.c_uint32(kmax), C.c_uint64(tick), _p(mask, C.c_uint8))
+    return mask
+
+
+def kick_rungs(vel4, acc_pot, rung, mask, dt_max):
+    assert vel4.dtype == np.float32 and vel4.flags.c_contiguous and vel4.shape[1] == 4
+    ap = _f32(acc_pot)
+    r = np.ascontiguousarray(rung, np.uint8)
+    m = None if mask is None else np.ascontiguousarray(mask, np.uint8)
+    lib().oracle_kick_rungs(_p(vel4, C.c_float), _p(ap, C.c_float), _p(r, C.c_uint8), _p(m, C.c_uint8),
+                            C.c_uint32(vel4.shape[0]), C.c_float(dt_max))
+
+
+def block_tick(pm, v4, ap, rung, tick, theta, eps, eta, dt_max, kmax, prev: Step = None, **kw):
+    """One tick of the block scheme (R27), in place on pm / v4 / ap / rung.  prev: refresh this Step's tree instead
+    of rebuilding (R25).  Returns (the Step of this tick, number of active particles walked)."""
+    m0 = active_at(rung, kmax, tick)
+    kick_rungs(v4, ap, rung, m0, dt_max)
+    drift(pm, v4, np.float32(np.ldexp(np.float32(dt_max), -kmax)))
+    m1 = active_at(rung, kmax, tick + 1)
+    if prev is None:
+        s = full_step(pm, theta, eps, active_mask=m1, **kw)
+    else:
+        s = refreshed_step(prev, pm, theta, eps, active_mask=m1, **kw)
+    sel = m1[s.perm].astype(bool)
+    new = np.empty((int(sel.sum()), 4), np.float64)
+    new[:, :3] = s.walk.acc[sel]
+    new[:, 3] = s.walk.pot[sel]
+    ap[s.perm[sel]] = new.astype(np.float32)
+    kick_rungs(v4, ap, rung, m1, dt_max)
+    rungs(ap, eta, eps, dt_max, kmax, rung=rung, mask=m1, tick=tick + 1)
+    return s, int(m1.sum())

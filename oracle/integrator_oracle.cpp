@@ -72,3 +72,66 @@ void oracle_diagnostics(const float* pos_mass, const float* vel4, const float* a
 }
 
 }  // extern "C"
+
+// =====================================================================================
+// Block time-steps (row f1/f2 of DESIGN.md; "block time-step algorithm", "N_active ... the number of
+// particles that have to be updated").  The paper gives no criterion or scheme.  Readings taken (R26, R27):
+//
+//   R26  Rungs.  Particle i steps with dt_i = dt_max 2^-k_i, k_i in [0, kmax] the SMALLEST k with
+//            dt_max 2^-k <= eta sqrt(eps / |a_i|)          (fp64 on the fp32 acceleration; |a| = 0 -> k = 0),
+//        clamped to kmax.  Time is counted in ticks of dt_min = dt_max 2^-kmax; i is ACTIVE at tick t iff
+//        t mod 2^(kmax - k_i) == 0 (its step ends / begins there).
+//   R27  One tick of the block scheme (kick-drift-kick per particle, every step aligned to its own rung):
+//          opening kick of the particles active at t:      v += a (dt_i / 2)
+//          drift of ALL particles:                          x += v dt_min
+//          force on the particles active at t + 1 (masked walk; tree rebuilt or refreshed, R25)
+//          closing kick of those:                           v += a_new (dt_i / 2)     (same rung as the opening kick)
+//          new rung for those from a_new: finer at once; coarser by ONE rung, and only if t + 1 is a multiple of
+//          the coarser step (so steps stay nested).
+//        Kicks are the fp32 fma of R23 with h = dt_max 2^-(k+1) (an exact power-of-two scaling).
+//        With kmax = 0 this is the shared-step leapfrog of R22, operation for operation.
+//
+// Pins (tests/test_oracle_integrator.py): rung formula against numpy; activity pattern and counts; kmax = 0
+// reproduces oracle.leapfrog bit for bit; rungs only coarsen at synchronised ticks; a Plummer core with block steps
+// conserves energy better than the shared dt_max step at a fraction of the force evaluations of the shared dt_min step.
+// =====================================================================================
+extern "C" {
+
+static uint32_t rung_of(const float* a, double eta, double eps, double dt_max, uint32_t kmax) {
+    const double ax = a[0], ay = a[1], az = a[2];
+    const double a2 = (ax * ax + ay * ay) + az * az;
+    if (!(a2 > 0.0)) return 0;
+    const double crit = eta * std::sqrt(eps / std::sqrt(a2));
+    uint32_t k = 0;
+    while (k < kmax && std::ldexp(dt_max, -(int)k) > crit) ++k;
+    return k;
+}
+
+// init != 0: rung[i] = R26 for every particle (mask ignored).  init == 0: the R27 update at `tick` for the particles
+// with mask[i] != 0 (mask null = all).
+void oracle_rungs(const float* acc_pot, uint32_t n, float eta, float eps, float dt_max, uint32_t kmax,
+                  const uint8_t* mask, uint64_t tick, uint8_t* rung, int init) {
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t want = rung_of(&acc_pot[4 * i], eta, eps, dt_max, kmax);
+        if (init) { rung[i] = (uint8_t)want; continue; }
+        if (mask && !mask[i]) continue;
+        const uint32_t cur = rung[i];
+        if (want > cur) rung[i] = (uint8_t)want;
+        else if (want < cur && (tick % (1ull << (kmax - (cur - 1)))) == 0) rung[i] = (uint8_t)(cur - 1);
+    }
+}
+
+void oracle_active_mask(const uint8_t* rung, uint32_t n, uint32_t kmax, uint64_t tick, uint8_t* mask) {
+    for (uint32_t i = 0; i < n; ++i) mask[i] = (tick % (1ull << (kmax - rung[i]))) == 0 ? 1 : 0;
+}
+
+// v_a <- fma(acc_a, dt_max 2^-(rung+1), v_a) for the particles with mask != 0 (null = all).
+void oracle_kick_rungs(float* vel4, const float* acc_pot, const uint8_t* rung, const uint8_t* mask, uint32_t n, float dt_max) {
+    for (uint32_t i = 0; i < n; ++i) {
+        if (mask && !mask[i]) continue;
+        const float h = std::ldexp(dt_max, -(int)rung[i] - 1);
+        for (int a = 0; a < 3; ++a) vel4[4 * i + a] = std::fmaf(acc_pot[4 * i + a], h, vel4[4 * i + a]);
+    }
+}
+
+}  // extern "C"

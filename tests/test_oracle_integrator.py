@@ -135,3 +135,84 @@ def test_tree_leapfrog_tracks_direct_leapfrog():
     pt, vt, _ = O.leapfrog(pm, vel, 0.5, 0.01, dt, 8)
     assert np.abs(pd[:, :3] - pt[:, :3]).max() < 1e-5
     assert np.abs(vd[:, :3] - vt[:, :3]).max() < 2e-3
+
+
+# ---- block time-steps (R26, R27) ------------------------------------------------------------------------
+
+def test_rung_formula_against_numpy_and_activity_pattern():
+    pm, vel = W.plummer(2048, with_velocities=True)
+    eps, eta, dt_max, kmax = 0.01, 0.02, 1.0 / 64, 5
+    ap = O.force_f32(pm, 0.0, eps)
+    r = O.rungs(ap, eta, eps, dt_max, kmax)
+    a = np.linalg.norm(ap[:, :3].astype(np.float64), axis=1)
+    crit = np.float64(np.float32(eta)) * np.sqrt(np.float64(np.float32(eps)) / a)
+    want = np.clip(np.ceil(np.log2(np.float64(np.float32(dt_max)) / crit)), 0, kmax).astype(np.int64)
+    assert (r == want).mean() > 0.999                     # log2 at an exact power of two may round either way
+    ok = r < kmax
+    assert np.all(np.ldexp(dt_max, -r[ok].astype(int)) <= crit[ok])           # the step satisfies the criterion ...
+    big = r > 0
+    assert np.all(np.ldexp(dt_max, -(r[big].astype(int) - 1)) > crit[big])    # ... and the next coarser one does not
+    assert len(np.unique(r)) >= 3                          # the core needs finer steps than the halo
+    for tick in (0, 1, 2, 4, 6, 16, 32):
+        m = O.active_at(r, kmax, tick)
+        assert np.array_equal(m.astype(bool), tick % (1 << (kmax - r.astype(int))) == 0)
+    assert O.active_at(r, kmax, 0).all() and O.active_at(r, kmax, 32).all()
+    assert O.active_at(r, kmax, 1).sum() == (r == kmax).sum()
+
+
+def test_block_scheme_with_one_rung_is_the_shared_leapfrog_bit_for_bit():
+    pm, vel = W.plummer(300, with_velocities=True)
+    theta, eps, dt = 0.5, 0.02, np.float32(1 / 128)
+    p_ref, v_ref, a_ref = O.leapfrog(pm, vel, theta, eps, dt, 5)
+    p, v = pm.copy(), O._vel4(vel)
+    ap = O.force_f32(p, theta, eps)
+    rung = np.zeros(300, np.uint8)
+    for tick in range(5):
+        O.block_tick(p, v, ap, rung, tick, theta, eps, 1e9, dt, 0)     # eta huge: nobody wants a finer rung
+    assert np.array_equal(p.view(np.uint32), p_ref.view(np.uint32))
+    assert np.array_equal(v.view(np.uint32), v_ref.view(np.uint32))
+    assert np.array_equal(ap.view(np.uint32), a_ref.view(np.uint32))
+
+
+def test_rungs_coarsen_only_at_synchronised_ticks():
+    n, kmax = 64, 4
+    ap = np.zeros((n, 4), np.float32)
+    ap[:, 0] = 1e-6                                       # tiny acceleration: every particle wants rung 0
+    rung = np.full(n, kmax, np.uint8)
+    history = []
+    for tick in range(1, 17):
+        mask = O.active_at(rung, kmax, tick)
+        before = rung.copy()
+        O.rungs(ap, 0.02, 0.01, 1 / 64, kmax, rung=rung, mask=mask, tick=tick)
+        changed = rung != before
+        assert np.all(before[changed] - rung[changed] == 1)                     # one rung at a time
+        assert np.all(tick % (1 << (kmax - rung[changed].astype(int))) == 0)    # aligned to the NEW, coarser step
+        assert not changed[mask == 0].any()
+        history.append(int(rung[0]))
+    assert history[0] == kmax and history[-1] == 0        # 4 -> 3 at tick 2, -> 2 at 4, -> 1 at 8, -> 0 at 16
+    assert history[1] == 3 and history[3] == 2 and history[7] == 1
+
+
+def test_block_steps_beat_the_coarse_shared_step_at_a_fraction_of_the_fine_cost():
+    n = 256
+    pm, vel = W.plummer(n, with_velocities=True)
+    eps, eta, dt_max, kmax = 0.005, 0.1, 1.0 / 32, 4      # rungs 0..3 populated: 7 / 23 / 108 / 118 particles
+
+    def energy(p, v, a):
+        d = O.diagnostics(p, v, a)
+        return d[0] + d[1]
+
+    a0 = O.force_f32(pm, 0.0, eps)
+    e0 = energy(pm, O._vel4(vel), a0)
+    pc, vc, ac = O.leapfrog(pm, vel, 0.0, eps, np.float32(dt_max), 4, acc_pot=a0)          # shared dt_max
+    err_coarse = abs(energy(pc, vc, ac) / e0 - 1)
+    p, v, ap = pm.copy(), O._vel4(vel), a0.copy()
+    rung = O.rungs(ap, eta, eps, dt_max, kmax)
+    walked = 0
+    for tick in range(4 << kmax):
+        _, na = O.block_tick(p, v, ap, rung, tick, 0.0, eps, eta, dt_max, kmax)
+        walked += na
+    assert O.active_at(rung, kmax, 4 << kmax).all()       # everybody is synchronised at a multiple of dt_max
+    err_block = abs(energy(p, v, O.force_f32(p, 0.0, eps)) / e0 - 1)
+    assert err_block < 0.1 * err_coarse                   # measured: 9.5e-8 against 4.7e-6
+    assert walked < 0.4 * n * (4 << kmax)                 # far fewer force evaluations than the shared dt_min step
