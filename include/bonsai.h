@@ -221,6 +221,36 @@ int bonsai_leapfrog_step(bonsai_ctx* ctx, float* pos_mass_dev, float* vel_dev, f
 int bonsai_diagnostics(bonsai_ctx* ctx, const float* pos_mass_dev, const float* vel_dev, const float* acc_pot_dev,
                        uint32_t n, double* out12_dev);
 
+/* ---- Block time-steps (R26, R27; "block time-step algorithm", "N_active") -----------------
+ * The paper states no criterion or scheme.  R26: particle i steps with dt_i = dt_max 2^-k_i, its rung k_i in
+ * [0, kmax] the smallest k with dt_max 2^-k <= eta sqrt(eps / |a_i|) (fp64 on the fp32 acceleration).  Time is
+ * counted in ticks of dt_min = dt_max 2^-kmax; i is active at tick t iff t mod 2^(kmax - k_i) == 0.  kmax <= 30.
+ * rung / mask arrays are device u8[n] in load order, caller-owned.  Asynchronous on the context's stream. */
+
+/* init != 0: rung[i] = R26 for every particle.  init == 0: the update at the end of a tick for the particles with
+ * mask != 0 (NULL = all): a finer rung at once, a coarser one by one rung and only if `tick` is a multiple of the
+ * coarser step (steps stay nested). */
+int bonsai_timestep_rungs(bonsai_ctx* ctx, const float* acc_pot_dev, uint32_t n, float eta, float eps, float dt_max,
+                          uint32_t kmax, const uint8_t* active_mask_dev, uint64_t tick, uint8_t* rung_dev, int init);
+
+/* mask[i] = 1 if particle i is active at `tick`, else 0: the mask bonsai_walk / bonsai_kick_rungs take. */
+int bonsai_active_mask(bonsai_ctx* ctx, const uint8_t* rung_dev, uint32_t n, uint32_t kmax, uint64_t tick,
+                       uint8_t* mask_dev_out);
+
+/* Half a step of each masked-in particle's own size: vel.xyz = fma(acc.xyz, dt_max 2^-(rung+1), vel.xyz) (R23). */
+int bonsai_kick_rungs(bonsai_ctx* ctx, float* vel_dev, const float* acc_pot_dev, const uint8_t* rung_dev,
+                      const uint8_t* active_mask_dev, uint32_t n, float dt_max);
+
+/* One tick of the block scheme (R27), everything on the device, no host read-back:
+ *   opening kick of the particles active at `tick`; drift of ALL particles by dt_min; force on the particles active
+ *   at tick + 1 (masked walk) from a rebuilt (rebuild != 0) or refreshed (rebuild == 0, bonsai_refresh_tree) tree;
+ *   closing kick of those; their new rungs.
+ * acc_pot_dev holds every particle's force at its last force time and is updated for the walked particles only.
+ * With kmax = 0 this is bonsai_leapfrog_step.  ESTATE if rebuild == 0 and no tree for this array / n exists. */
+int bonsai_block_tick(bonsai_ctx* ctx, float* pos_mass_dev, float* vel_dev, float* acc_pot_dev, uint8_t* rung_dev,
+                      uint32_t n, uint64_t tick, float theta, float eps, float eta, float dt_max, uint32_t kmax,
+                      int rebuild);
+
 /* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events between stages from then on;
  * bonsai_get_stage_ms() waits for the stream and writes milliseconds of the most recent execution of each
  * stage: 0 bbox, 1 keys, 2 sort, 3 reorder, 4 build, 5 groups, 6 multipoles, 7 walk, 8 integrate (the most

@@ -30,6 +30,7 @@ SYMBOLS = (
     "bonsai_get_counts", "bonsai_get_interaction_totals", "bonsai_set_timing", "bonsai_get_stage_ms",
     "bonsai_get_launch_count", "bonsai_strerror",
     "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
+    "bonsai_timestep_rungs", "bonsai_active_mask", "bonsai_kick_rungs", "bonsai_block_tick",
 )
 
 
@@ -89,6 +90,11 @@ def lib() -> C.CDLL:
     L.bonsai_get_launch_count.argtypes = [vp]
     L.bonsai_get_launch_count.restype = C.c_uint64
     L.bonsai_refresh_tree.argtypes = [vp]
+    u64 = C.c_uint64
+    L.bonsai_timestep_rungs.argtypes = [vp, vp, u32, f32, f32, f32, u32, vp, u64, vp, C.c_int]
+    L.bonsai_active_mask.argtypes = [vp, vp, u32, u32, u64, vp]
+    L.bonsai_kick_rungs.argtypes = [vp, vp, vp, vp, vp, u32, f32]
+    L.bonsai_block_tick.argtypes = [vp, vp, vp, vp, vp, u32, u64, f32, f32, f32, f32, u32, C.c_int]
     L.bonsai_kick.argtypes = [vp, vp, vp, u32, f32, vp]
     L.bonsai_drift.argtypes = [vp, vp, vp, u32, f32]
     L.bonsai_leapfrog_step.argtypes = [vp, vp, vp, vp, u32, f32, f32, f32]
@@ -286,6 +292,55 @@ class Bonsai:
             _check(self._L.bonsai_diagnostics(self._h, self._f4(pos_mass), self._f4(vel, n), self._f4(acc_pot, n), n,
                                               out.data_ptr()), "bonsai_diagnostics")
         return out
+
+    # ---- block time-steps (R26, R27) ----------------------------------------------------------------
+    @staticmethod
+    def _u8(t: torch.Tensor, n: int) -> int:
+        assert t.is_cuda and t.dtype == torch.uint8 and t.is_contiguous() and t.numel() == n
+        return t.data_ptr()
+
+    def timestep_rungs(self, acc_pot: torch.Tensor, eta: float, eps: float, dt_max: float, kmax: int,
+                       rung: torch.Tensor | None = None, active_mask: torch.Tensor | None = None,
+                       tick: int = 0) -> torch.Tensor:
+        """rung is None: fresh assignment (R26) -> uint8[n] device tensor; else the end-of-tick update in place."""
+        n = acc_pot.shape[0]
+        init = rung is None
+        if init:
+            rung = torch.zeros(n, dtype=torch.uint8, device=self.device)
+        mptr = None if active_mask is None else self._u8(active_mask, n)
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_timestep_rungs(self._h, self._f4(acc_pot), n, float(eta), float(eps), float(dt_max),
+                                                 int(kmax), mptr, int(tick), self._u8(rung, n), int(init)),
+                   "bonsai_timestep_rungs")
+        return rung
+
+    def active_mask(self, rung: torch.Tensor, kmax: int, tick: int, out: torch.Tensor | None = None) -> torch.Tensor:
+        n = rung.numel()
+        if out is None:
+            out = torch.zeros(n, dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_active_mask(self._h, self._u8(rung, n), n, int(kmax), int(tick), self._u8(out, n)),
+                   "bonsai_active_mask")
+        return out
+
+    def kick_rungs(self, vel: torch.Tensor, acc_pot: torch.Tensor, rung: torch.Tensor,
+                   active_mask: torch.Tensor | None, dt_max: float) -> None:
+        n = vel.shape[0]
+        mptr = None if active_mask is None else self._u8(active_mask, n)
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_kick_rungs(self._h, self._f4(vel), self._f4(acc_pot, n), self._u8(rung, n), mptr, n,
+                                             float(dt_max)), "bonsai_kick_rungs")
+
+    def block_tick(self, pos_mass: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor, rung: torch.Tensor, tick: int,
+                   theta: float, eps: float, eta: float, dt_max: float, kmax: int, rebuild: bool = True) -> None:
+        """One tick of the block time-step scheme in place (bonsai_block_tick)."""
+        n = pos_mass.shape[0]
+        self._keep = [pos_mass]
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_block_tick(self._h, self._f4(pos_mass), self._f4(vel, n), self._f4(acc_pot, n),
+                                             self._u8(rung, n), n, int(tick), float(theta), float(eps), float(eta),
+                                             float(dt_max), int(kmax), int(bool(rebuild))), "bonsai_block_tick")
+        self.n = n
 
     def sync(self) -> None:
         _check(self._L.bonsai_sync(self._h), "bonsai_sync")

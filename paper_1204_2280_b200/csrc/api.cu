@@ -103,6 +103,7 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     t.host_in = cv.take<float4>(n);
     t.host_out = cv.take<float4>(n);
     t.host_mask = cv.take<uint8_t>(n);
+    t.tick_mask = cv.take<uint8_t>(n);
     if (b) *b = t;
     return (cv.off + kAlign - 1) / kAlign * kAlign;
 }
@@ -336,6 +337,72 @@ int bonsai_leapfrog_step(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, flo
         BONSAI_TRY(stage_kick(c, reinterpret_cast<float4*>(vel_dev), reinterpret_cast<const float4*>(acc_pot_dev), n, half,
                               nullptr));
     }
+    return BONSAI_OK;
+}
+
+// ---- block time-steps (R26, R27) --------------------------------------------------------------------------
+
+int bonsai_timestep_rungs(bonsai_ctx* h, const float* acc_pot_dev, uint32_t n, float eta, float eps, float dt_max,
+                          uint32_t kmax, const uint8_t* active_mask_dev, uint64_t tick, uint8_t* rung_dev, int init) {
+    if (!h || !acc_pot_dev || !rung_dev || !aligned16(acc_pot_dev)) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max || kmax > 30u) return BONSAI_EINVAL;
+    if (!(eta > 0.0f) || !(eps > 0.0f) || !(dt_max > 0.0f) || std::isinf(eta) || std::isinf(eps) || std::isinf(dt_max))
+        return BONSAI_EINVAL;
+    BONSAI_TRY(stage_rungs(&h->c, reinterpret_cast<const float4*>(acc_pot_dev), n, eta, eps, dt_max, kmax, active_mask_dev,
+                           tick, rung_dev, init));
+    return BONSAI_OK;
+}
+
+int bonsai_active_mask(bonsai_ctx* h, const uint8_t* rung_dev, uint32_t n, uint32_t kmax, uint64_t tick,
+                       uint8_t* mask_dev_out) {
+    if (!h || !rung_dev || !mask_dev_out) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max || kmax > 30u) return BONSAI_EINVAL;
+    BONSAI_TRY(stage_active_mask(&h->c, rung_dev, n, kmax, tick, mask_dev_out));
+    return BONSAI_OK;
+}
+
+int bonsai_kick_rungs(bonsai_ctx* h, float* vel_dev, const float* acc_pot_dev, const uint8_t* rung_dev,
+                      const uint8_t* active_mask_dev, uint32_t n, float dt_max) {
+    if (!h || !vel_dev || !acc_pot_dev || !rung_dev || !aligned16(vel_dev) || !aligned16(acc_pot_dev)) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max || !std::isfinite(dt_max)) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    StageTimer t(c, 8);
+    BONSAI_TRY(stage_kick_rungs(c, reinterpret_cast<float4*>(vel_dev), reinterpret_cast<const float4*>(acc_pot_dev), rung_dev,
+                                active_mask_dev, n, dt_max));
+    return BONSAI_OK;
+}
+
+int bonsai_block_tick(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, float* acc_pot_dev, uint8_t* rung_dev, uint32_t n,
+                      uint64_t tick, float theta, float eps, float eta, float dt_max, uint32_t kmax, int rebuild) {
+    if (!h || !pos_mass_dev || !vel_dev || !acc_pot_dev || !rung_dev) return BONSAI_EINVAL;
+    if (!aligned16(pos_mass_dev) || !aligned16(vel_dev) || !aligned16(acc_pot_dev)) return BONSAI_EINVAL;
+    if (n == 0 || n > h->c.n_max || kmax > 30u) return BONSAI_EINVAL;
+    if (!(theta >= 0.0f) || std::isinf(theta) || !(eta > 0.0f) || !(eps > 0.0f) || !(dt_max > 0.0f) || std::isinf(eta) ||
+        std::isinf(eps) || std::isinf(dt_max))
+        return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    if (!rebuild && (c->tree_n != n || c->pos_mass != reinterpret_cast<const float4*>(pos_mass_dev))) return BONSAI_ESTATE;
+    float4* vel = reinterpret_cast<float4*>(vel_dev);
+    const float4* acc = reinterpret_cast<const float4*>(acc_pot_dev);
+    uint8_t* mask = c->b.tick_mask;
+    const float dt_min = std::ldexp(dt_max, -(int)kmax);
+    int rc;
+    BONSAI_TRY(stage_active_mask(c, rung_dev, n, kmax, tick, mask));
+    {
+        StageTimer t(c, 8);
+        BONSAI_TRY(stage_kick_rungs(c, vel, acc, rung_dev, mask, n, dt_max));
+        BONSAI_TRY(stage_drift(c, reinterpret_cast<float4*>(pos_mass_dev), vel, n, dt_min));
+    }
+    BONSAI_TRY(stage_active_mask(c, rung_dev, n, kmax, tick + 1, mask));
+    if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
+    if ((rc = rebuild ? bonsai_build_tree(h) : bonsai_refresh_tree(h)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
+    if ((rc = bonsai_walk(h, theta, eps, mask, acc_pot_dev)) != BONSAI_OK) return rc;
+    {
+        StageTimer t(c, 8);
+        BONSAI_TRY(stage_kick_rungs(c, vel, acc, rung_dev, mask, n, dt_max));
+    }
+    BONSAI_TRY(stage_rungs(c, acc, n, eta, eps, dt_max, kmax, mask, tick + 1, rung_dev, 0));
     return BONSAI_OK;
 }
 

@@ -114,6 +114,79 @@ __global__ void __launch_bounds__(kDiagThreads) k_diagnostics(const float4* __re
     if (threadIdx.x == 0) ctl->diag_ticket = 0;  // ready for the next call
 }
 
+// ---- block time-steps (R26, R27) -----------------------------------------------------------------------
+// Rung of a particle: the smallest k with dt_max 2^-k <= eta sqrt(eps / |a|), fp64 on the fp32 acceleration, every
+// operation rounded once in the order written (no contraction), clamped to kmax.
+__device__ __forceinline__ uint32_t rung_of(const float4 a, double eta, double eps, double dt_max, uint32_t kmax) {
+    const double ax = a.x, ay = a.y, az = a.z;
+    const double a2 = __dadd_rn(__dadd_rn(__dmul_rn(ax, ax), __dmul_rn(ay, ay)), __dmul_rn(az, az));
+    if (!(a2 > 0.0)) return 0u;
+    const double crit = __dmul_rn(eta, sqrt(eps / sqrt(a2)));
+    uint32_t k = 0;
+    while (k < kmax && ldexp(dt_max, -(int)k) > crit) ++k;
+    return k;
+}
+
+__global__ void __launch_bounds__(256) k_rungs(const float4* __restrict__ acc, uint32_t n, float eta, float eps,
+                                               float dt_max, uint32_t kmax, const uint8_t* __restrict__ mask,
+                                               unsigned long long tick, uint8_t* __restrict__ rung, int init) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (!init && mask && !mask[i]) return;
+    const uint32_t want = rung_of(__ldg(&acc[i]), (double)eta, (double)eps, (double)dt_max, kmax);
+    if (init) {
+        rung[i] = (uint8_t)want;
+        return;
+    }
+    const uint32_t cur = rung[i];
+    if (want > cur) rung[i] = (uint8_t)want;                                          // finer at once
+    else if (want < cur && (tick % (1ull << (kmax - (cur - 1u)))) == 0ull) rung[i] = (uint8_t)(cur - 1u);  // nested
+}
+
+__global__ void __launch_bounds__(256) k_active_mask(const uint8_t* __restrict__ rung, uint32_t n, uint32_t kmax,
+                                                     unsigned long long tick, uint8_t* __restrict__ mask) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    mask[i] = ((tick % (1ull << (kmax - rung[i]))) == 0ull) ? 1 : 0;
+}
+
+// v <- fma(a, dt_max 2^-(rung+1), v) for the masked-in particles: half a step of the particle's own size.
+__global__ void __launch_bounds__(256) k_kick_rungs(float4* __restrict__ vel, const float4* __restrict__ acc,
+                                                    const uint8_t* __restrict__ rung, const uint8_t* __restrict__ mask,
+                                                    uint32_t n, float dt_max) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (mask && !mask[i]) return;
+    const float h = ldexpf(dt_max, -(int)rung[i] - 1);
+    float4 v = vel[i];
+    const float4 a = __ldg(&acc[i]);
+    v.x = __fmaf_rn(a.x, h, v.x);
+    v.y = __fmaf_rn(a.y, h, v.y);
+    v.z = __fmaf_rn(a.z, h, v.z);
+    vel[i] = v;
+}
+
+cudaError_t stage_rungs(Ctx* c, const float4* acc, uint32_t n, float eta, float eps, float dt_max, uint32_t kmax,
+                        const uint8_t* mask, unsigned long long tick, uint8_t* rung, int init) {
+    k_rungs<<<div_up(n, 256), 256, 0, c->stream>>>(acc, n, eta, eps, dt_max, kmax, mask, tick, rung, init);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t stage_active_mask(Ctx* c, const uint8_t* rung, uint32_t n, uint32_t kmax, unsigned long long tick,
+                              uint8_t* mask) {
+    k_active_mask<<<div_up(n, 256), 256, 0, c->stream>>>(rung, n, kmax, tick, mask);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t stage_kick_rungs(Ctx* c, float4* vel, const float4* acc, const uint8_t* rung, const uint8_t* mask,
+                             uint32_t n, float dt_max) {
+    k_kick_rungs<<<div_up(n, 256), 256, 0, c->stream>>>(vel, acc, rung, mask, n, dt_max);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
 cudaError_t stage_kick(Ctx* c, float4* vel, const float4* acc, uint32_t n, float h, const uint8_t* mask) {
     k_kick<<<div_up(n, 256), 256, 0, c->stream>>>(vel, acc, n, h, mask);
     c->launches += 1;

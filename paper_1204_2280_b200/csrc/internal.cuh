@@ -118,6 +118,7 @@ struct Buffers {
     // staging of bonsai_step_host
     float4 *host_in, *host_out;
     uint8_t* host_mask;
+    uint8_t* tick_mask;        // [n] active mask of bonsai_block_tick
 };
 
 struct Ctx {
@@ -158,6 +159,12 @@ size_t walk_smem_bytes(uint32_t nleaf);
 cudaError_t stage_kick(Ctx* c, float4* vel, const float4* acc, uint32_t n, float h, const uint8_t* mask);
 cudaError_t stage_drift(Ctx* c, float4* pos, const float4* vel, uint32_t n, float h);
 cudaError_t stage_kick_drift(Ctx* c, float4* pos, float4* vel, const float4* acc, uint32_t n, float hk, float hd);
+cudaError_t stage_rungs(Ctx* c, const float4* acc, uint32_t n, float eta, float eps, float dt_max, uint32_t kmax,
+                        const uint8_t* mask, unsigned long long tick, uint8_t* rung, int init);
+cudaError_t stage_active_mask(Ctx* c, const uint8_t* rung, uint32_t n, uint32_t kmax, unsigned long long tick,
+                              uint8_t* mask);
+cudaError_t stage_kick_rungs(Ctx* c, float4* vel, const float4* acc, const uint8_t* rung, const uint8_t* mask,
+                             uint32_t n, float dt_max);
 cudaError_t stage_diagnostics(Ctx* c, const float4* pos, const float4* vel, const float4* acc, uint32_t n, double* out);
 
 // Device-wide exclusive scan of u32 (scan.cu): out[i] = sum_{j<i} in[j], i in [0, n]; out has n+1 entries

@@ -1,0 +1,120 @@
+"""Parity of the block time-step calls (integrate.cu / bonsai_block_tick through the C-ABI binding) against the
+oracle (oracle/integrator_oracle.cpp R26-R27, oracle.block_tick).
+
+Gates: rungs, active masks and rung kicks BIT-EXACT; a run of block ticks (tree rebuilt, then refreshed) keeps the
+rung arrays identical to the oracle's and the trajectories within the walk's tolerance; one rung reproduces
+bonsai_leapfrog_step bit for bit."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle as O  # noqa: E402
+from paper_1204_2280_b200 import Bonsai, BonsaiError  # noqa: E402
+from paper_1204_2280_b200 import workloads as W  # noqa: E402
+from paper_1204_2280_b200.bonsai import EINVAL, ESTATE  # noqa: E402
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.mark.parametrize("n", [1, 257, 40001])
+def test_rungs_masks_kicks_bit_exact(n):
+    rng = np.random.default_rng(n)
+    ap = (rng.normal(size=(n, 4)) * np.exp(rng.normal(size=(n, 1)) * 3)).astype(np.float32)
+    ap[0, :3] = 0                                          # |a| = 0 -> rung 0
+    v = rng.normal(size=(n, 4)).astype(np.float32)
+    eta, eps, dt_max, kmax = 0.05, 0.01, 1 / 32, 6
+    b = Bonsai(n)
+    ap_d = _dev(ap)
+    r_d = b.timestep_rungs(ap_d, eta, eps, dt_max, kmax)
+    r = O.rungs(ap, eta, eps, dt_max, kmax)
+    assert np.array_equal(r_d.cpu().numpy(), r)
+    if n > 1:
+        assert len(np.unique(r)) >= 4
+    for tick in (0, 1, 2, 3, 8, 24, 64):
+        m = O.active_at(r, kmax, tick)
+        m_d = b.active_mask(r_d, kmax, tick)
+        assert np.array_equal(m_d.cpu().numpy(), m)
+        v_d = _dev(v)
+        b.kick_rungs(v_d, ap_d, r_d, m_d, dt_max)
+        v_ref = v.copy(); O.kick_rungs(v_ref, ap, r, m, np.float32(dt_max))
+        assert np.array_equal(v_d.cpu().numpy().view(np.uint32), v_ref.view(np.uint32))
+        # end-of-tick update with different accelerations
+        ap2 = (ap * np.float32(0.05 + 3.0 * ((tick + 1) % 3))).astype(np.float32)
+        r2 = r.copy(); O.rungs(ap2, eta, eps, dt_max, kmax, rung=r2, mask=m, tick=tick)
+        r2_d = r_d.clone(); b.timestep_rungs(_dev(ap2), eta, eps, dt_max, kmax, rung=r2_d, active_mask=m_d, tick=tick)
+        assert np.array_equal(r2_d.cpu().numpy(), r2)
+
+
+def test_one_rung_is_leapfrog_step_bit_for_bit():
+    n, theta, eps, dt = 5000, 0.6, 0.02, 1 / 256
+    pm, vel = W.plummer(n, with_velocities=True)
+    b = Bonsai(n)
+    pa, va = _dev(pm), _dev(O._vel4(vel))
+    aa = b.step(pa, theta, eps).clone()
+    pb, vb, ab = pa.clone(), va.clone(), aa.clone()
+    rung = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    for t in range(3):
+        b.leapfrog_step(pa, va, aa, theta, eps, dt)
+        b.block_tick(pb, vb, ab, rung, t, theta, eps, 1e9, dt, 0, rebuild=True)
+    b.sync()
+    for x, y in ((pa, pb), (va, vb), (aa, ab)):
+        assert np.array_equal(x.cpu().numpy().view(np.uint32), y.cpu().numpy().view(np.uint32))
+    assert int(rung.max()) == 0
+
+
+@pytest.mark.parametrize("rebuild_every", [1, 4])
+def test_block_ticks_follow_the_oracle(rebuild_every):
+    n, theta, eps, eta, dt_max, kmax = 8192, 0.75, 0.01, 0.1, 1 / 32, 3
+    pm, vel = W.plummer(n, with_velocities=True)
+    b = Bonsai(n)
+    p_d, v_d = _dev(pm), _dev(O._vel4(vel))
+    a_d = b.step(p_d, theta, eps).clone()
+    r_d = b.timestep_rungs(a_d, eta, eps, dt_max, kmax)
+    p, v = pm.copy(), O._vel4(vel)
+    ap = O.force_f32(p, theta, eps)
+    r = O.rungs(ap, eta, eps, dt_max, kmax)
+    assert np.array_equal(r_d.cpu().numpy(), r) or (r_d.cpu().numpy() != r).mean() < 1e-3
+    r = r_d.cpu().numpy().copy()                          # start both sides from the same rungs
+    prev = None
+    walked = 0
+    for tick in range(8):
+        rebuild = tick % rebuild_every == 0
+        b.block_tick(p_d, v_d, a_d, r_d, tick, theta, eps, eta, dt_max, kmax, rebuild=rebuild)
+        s, na = O.block_tick(p, v, ap, r, tick, theta, eps, eta, dt_max, kmax, prev=None if rebuild else prev)
+        prev = s
+        walked += na
+        # rungs flip only where |a| sits on a rung boundary within the walk's tolerance
+        assert (r_d.cpu().numpy() != r).mean() < 2e-3
+        r = r_d.cpu().numpy().copy()
+    b.sync()
+    assert walked < 0.7 * 8 * n                           # a real block scheme: not everybody every tick
+    pg, vg = p_d.cpu().numpy(), v_d.cpu().numpy()
+    assert np.array_equal(pg[:, 3], pm[:, 3])
+    dx = np.abs(pg[:, :3].astype(np.float64) - p[:, :3])
+    dv = np.abs(vg[:, :3].astype(np.float64) - v[:, :3])
+    vrms = np.sqrt(np.mean(vel.astype(np.float64) ** 2))
+    assert np.median(dx) <= 2e-7 and np.quantile(dx, 0.999) <= 1e-5
+    assert np.median(dv) <= 1e-6 * vrms and np.quantile(dv, 0.999) <= 1e-3 * vrms
+
+
+def test_block_tick_errors():
+    n = 1000
+    pm, vel = W.plummer(n, with_velocities=True)
+    b = Bonsai(n)
+    p_d, v_d = _dev(pm), _dev(O._vel4(vel))
+    a_d = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+    r_d = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    with pytest.raises(BonsaiError) as e:                 # no tree yet: a refresh is impossible
+        b.block_tick(p_d, v_d, a_d, r_d, 0, 0.75, 0.01, 0.1, 1 / 32, 2, rebuild=False)
+    assert e.value.code == ESTATE
+    with pytest.raises(BonsaiError) as e:
+        b.block_tick(p_d, v_d, a_d, r_d, 0, 0.75, 0.01, 0.1, 1 / 32, 31, rebuild=True)
+    assert e.value.code == EINVAL
+    b.block_tick(p_d, v_d, a_d, r_d, 0, 0.75, 0.01, 0.1, 1 / 32, 2, rebuild=True)
+    b.block_tick(p_d, v_d, a_d, r_d, 1, 0.75, 0.01, 0.1, 1 / 32, 2, rebuild=False)
+    b.sync()
