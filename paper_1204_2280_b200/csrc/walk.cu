@@ -553,8 +553,11 @@ cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
     // reset the ticket and the interaction totals (adjacent fields of the control block)
     if ((e = cudaMemsetAsync(&b.ctl->walk_ticket, 0, sizeof(uint32_t), c->stream)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(&b.ctl->sum_pp, 0, 2 * sizeof(unsigned long long), c->stream)) != cudaSuccess) return e;
-    // a masked walk may have far fewer groups than resident warps: the team-capable kernel adapts on the device
-    const int which = ((a.eps2 == 0.0f) ? 1 : 0) + (c->groups_all_active ? 0 : 2);
+    // a masked walk, or a small system, may have far fewer groups than resident warps: the team-capable kernel
+    // adapts on the device; n / ncrit is a lower bound of the all-active group count known on the host
+    const unsigned long long resident_warps = (unsigned long long)c->num_sms * max(1, blocks_per_sm[2]) * kWalkWarps;
+    const bool few_groups = !c->groups_all_active || 2ull * (c->n / c->prm.ncrit) <= resident_warps;
+    const int which = ((a.eps2 == 0.0f) ? 1 : 0) + (few_groups ? 2 : 0);
     const int grid = c->num_sms * max(1, blocks_per_sm[which]);
     kernels[which]<<<grid, kWalkWarps * 32, smem, c->stream>>>(a);
     c->launches += 1;
