@@ -184,11 +184,14 @@ __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ gh
 }
 
 // ------------------------------------------------------------------------------------------------
-// a2  Stable LSD radix sort of (90-bit key, index) records (R5): 9 passes of 10-bit digits, lo word
-// first.  Only (current 30-bit word, index) PAIRS move: a pass reads 8 B and writes 8 B per particle.
-// When the passes of one word are done the next word is fetched through the index (passes 3 and 6
-// gather mid[idx], hi[idx] from the load-order key arrays); the sorted 90-bit keys are re-derived from
-// the reordered positions in k_reorder (a key is a pure function of the position and the root cube).
+// a2  Stable radix sort of (90-bit key, index) records (R5).  LSD passes of 10-bit digits over (current
+// 30-bit word, index) PAIRS: a pass reads 8 B and writes 8 B per particle.  When the passes of one word are
+// done the next word is fetched through the index (gather from the load-order key arrays); the sorted
+// 90-bit keys are re-derived from the reordered positions in k_reorder (a key is a pure function of the
+// position and the root cube).  The sort proper runs SIX passes, over the mid and hi words: the lo word
+// (levels 21-30) almost never decides the order, and k_sort_ties repairs the runs of equal (hi, mid)
+// after the reorder; the full nine-pass chain (lo word first) stays enqueued behind a device flag for
+// inputs with long runs (see stage_sort_ties).
 //
 // One kernel per pass, single sweep with decoupled look-back:
 //   * tiles of kSortTile pairs are handed out by an atomic ticket, so a tile's predecessors have
