@@ -345,6 +345,40 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
 #pragma unroll
     for (int k = 0; k < kWarps; ++k)
         if (k < w) tstart += s_wsum[k];
+    // The tile's aggregates are out; everything that only needs tile-local information comes BEFORE the look-back
+    // (first slot of each digit, slot of every pair, staging into shared memory), so the predecessors get that much
+    // more time to publish and the wait below is that much shorter.
+    {
+        uint32_t ts = tstart;
+#pragma unroll
+        for (int q = 0; q < kDig; ++q) {
+            s_tstart[d0 + q] = ts;
+            ts += tot[q];
+        }
+    }
+    __syncthreads();
+
+    // tile-sorted slot of every pair (the counters now hold the exclusive prefix over warps)
+#pragma unroll
+    for (int r = 0; r < kSortItems; ++r) {
+        const bool valid = base_w + r * 32 + l < a.n;
+        if (valid) {
+            const uint32_t d = (key[r] >> a.shift) & (kRadix - 1);
+            rnk[r] += s_tstart[d] + cnt[d];
+        }
+    }
+    __syncthreads();  // counters are dead: reuse them as the staging area
+    uint32_t* s_key = smem;
+    uint32_t* s_idx = smem + kSortTile;
+#pragma unroll
+    for (int r = 0; r < kSortItems; ++r) {
+        const uint32_t i = base_w + r * 32 + l;
+        if (i < a.n) {
+            s_key[rnk[r]] = key[r];
+            s_idx[rnk[r]] = (MODE == 0) ? i : __ldg(&a.idx_in[i]);
+        }
+    }
+
     // decoupled look-back, all of the thread's digits in flight together
     uint32_t excl[kDig];
 #pragma unroll
@@ -390,31 +424,8 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
     }
 #pragma unroll
     for (int q = 0; q < kDig; ++q) {
-        s_tstart[d0 + q] = tstart;
         s_gdst[d0 + q] = __ldg(&a.gbase[d0 + q]) + excl[q] - tstart;
         tstart += tot[q];
-    }
-    __syncthreads();
-
-    // tile-sorted slot of every pair (the counters now hold the exclusive prefix over warps)
-#pragma unroll
-    for (int r = 0; r < kSortItems; ++r) {
-        const bool valid = base_w + r * 32 + l < a.n;
-        if (valid) {
-            const uint32_t d = (key[r] >> a.shift) & (kRadix - 1);
-            rnk[r] += s_tstart[d] + cnt[d];
-        }
-    }
-    __syncthreads();  // counters are dead: reuse them as the staging area
-    uint32_t* s_key = smem;
-    uint32_t* s_idx = smem + kSortTile;
-#pragma unroll
-    for (int r = 0; r < kSortItems; ++r) {
-        const uint32_t i = base_w + r * 32 + l;
-        if (i < a.n) {
-            s_key[rnk[r]] = key[r];
-            s_idx[rnk[r]] = (MODE == 0) ? i : __ldg(&a.idx_in[i]);
-        }
     }
     __syncthreads();
     const uint32_t tile_base = tile * kSortTile;

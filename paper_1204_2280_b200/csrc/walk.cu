@@ -463,7 +463,8 @@ __device__ __forceinline__ void walk_groups(WarpSmem& S, const WalkArgs& a, uint
         if (kTeam) {
             if (slot == 0 && lane == 0) s_team_g[team] = atomicAdd(&a.ctl->walk_ticket, 1u);
             team_barrier(team, tsize);
-            g = s_team_g[team];  // the next write is behind the barriers at the end of walk_chunk
+            g = s_team_g[team];
+            team_barrier(team, tsize);  // everybody has read it before member 0 can draw the next ticket
         } else {
             if (lane == 0) g = atomicAdd(&a.ctl->walk_ticket, 1u);
             g = __shfl_sync(0xFFFFFFFFu, g, 0);
