@@ -5,6 +5,7 @@
   configs[4]  N = 2^20: walk of an active subset (N/16, N/256; scattered and clustered) against the full walk,
               with the tree rebuilt and with the tree refreshed (bonsai_refresh_tree)
   scaling     N = 2^15 ... 2^22: time per stage (the paper's Fig. 2 quantity)
+  merger      N = 2^20: the second workload (two Plummer spheres on approach) against the single sphere
 
 Everything runs through the C-ABI binding on cuda:0 with seeded synthetic Plummer spheres; times are CUDA-event
 stage times of the library (median of `--reps`), L2 not flushed between repetitions.  Prints one JSON document.
@@ -133,14 +134,34 @@ def scaling(reps: int) -> dict:
     return rows
 
 
+def merger(reps: int) -> dict:
+    """Second workload: two Plummer spheres (mass ratio 3) on approach, N = 2^20, against the single sphere."""
+    n, eps, theta = 1 << 20, 0.0025, 0.75
+    res = {}
+    for name, pm_h in (("plummer", W.plummer(n)), ("merger", W.merger(n)[0])):
+        pm = torch.from_numpy(pm_h).cuda()
+        b = Bonsai(n)
+        b.set_timing(True)
+        b.step(pm, theta, eps)
+        b.sync()
+        st = _median_stage(b, lambda: b.step(pm, theta, eps), reps)
+        pp, pc = b.interaction_totals()
+        st.pop("integrate", None)
+        res[name] = {"step_ms": sum(st.values()), "walk_ms": st["walk"], "pp_per_particle": pp / n,
+                     "pc_per_particle": pc / n, "n_cells": b.cells(False).n_cells, "n_groups": b.groups().n_groups}
+        del b
+    return {"n": n, "eps": eps, "theta": theta, "by_workload": res}
+
+
 def main() -> None:
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--reps", type=int, default=5)
-    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling"), default=None)
+    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling", "merger"), default=None)
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("report: no CUDA device -- libbonsai has no CPU fallback")
-    parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "scaling": scaling}
+    parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "scaling": scaling,
+             "merger": merger}
     doc = {k: f(args.reps) for k, f in parts.items() if args.only in (None, k)}
     print(json.dumps(doc, indent=1))
 

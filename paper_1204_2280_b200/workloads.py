@@ -118,6 +118,44 @@ def plummer(n: int, seed: int = SEED_PARTICLES, with_velocities: bool = False,
     return pos_mass, np.ascontiguousarray(vel.astype(np.float32))
 
 
+def merger(n: int, separation: float = 6.0, mass_ratio: float = 3.0, approach_speed: float = 0.4,
+           seed: int = SEED_PARTICLES):
+    """Second workload (DESIGN.md row f4; P:L56 lists other uses of the tree): two Plummer spheres
+    on a head-on approach -- an asymmetric, two-centred system that stresses group quality and the root cube.
+
+    Sphere A holds mass_ratio / (1 + mass_ratio) of the particles and of the mass, sphere B the rest, scaled to
+    sqrt(mass fraction) of A's radius; centres at -+ separation / 2 along x weighted so the centre of mass is at the
+    origin, relative speed ``approach_speed`` along x.  Particles of B continue A's counter stream (index n_a ...).
+    Returns (pos_mass float32[n, 4], vel float32[n, 3]); total mass 1.
+    """
+    if n < 2:
+        raise ValueError("n must be at least 2")
+    fa = mass_ratio / (1.0 + mass_ratio)
+    n_a = min(max(int(round(n * fa)), 1), n - 1)
+    n_b = n - n_a
+    pa, va = plummer(n_a, seed, with_velocities=True)
+    pb, vb = plummer(n_b, seed, with_velocities=True, first=n_a)
+    ma, mb = n_a / n, n_b / n
+    pa = pa.astype(np.float64); pb = pb.astype(np.float64)
+    va = va.astype(np.float64); vb = vb.astype(np.float64)
+    pa[:, 3] = 1.0 / n
+    pb[:, 3] = 1.0 / n
+    # a Plummer sphere of mass M and radius scale R has velocities ~ sqrt(M / R); B is smaller by sqrt(mb / ma) in radius
+    sb = np.sqrt(mb / ma)
+    pa[:, :3] *= 1.0                       # A keeps the Henon-unit scale of the generator (mass rescaled below)
+    va *= np.sqrt(ma)
+    pb[:, :3] *= sb
+    vb *= np.sqrt(mb / sb)
+    xa, xb = -separation * mb, separation * ma          # centre of mass at the origin
+    pa[:, 0] += xa
+    pb[:, 0] += xb
+    va[:, 0] += approach_speed * mb
+    vb[:, 0] -= approach_speed * ma
+    pos = np.concatenate([pa, pb]).astype(np.float32)
+    vel = np.concatenate([va, vb]).astype(np.float32)
+    return np.ascontiguousarray(pos), np.ascontiguousarray(vel)
+
+
 def active_mask(pos_mass: np.ndarray, n_active: int, pattern: str = "scattered",
                 seed: int = SEED_ACTIVE) -> np.ndarray:
     """uint8[n] mask in LOAD order with exactly ``n_active`` ones (BASELINE.json configs[4]).

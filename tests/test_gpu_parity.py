@@ -256,6 +256,18 @@ def test_sort_ties_below_the_20th_level(clump_sizes):
     check_walk(b, out, ref, count_frac=0.98, eps=0.01, pm=pm)
 
 
+@pytest.mark.parametrize("mode", [2, 0])
+def test_merger_workload(mode):
+    """Second workload (row f4): two Plummer spheres of mass ratio 3 on approach -- two density centres, a root cube
+    that is mostly empty, groups of very different extent."""
+    pm, _ = W.merger(60_001)
+    ref = O.full_step(pm, 0.75, 0.005, group_mode=mode)
+    b, out = run_gpu(pm, 0.75, 0.005, group_mode=mode)
+    check_structure(b, ref)
+    check_groups(b, ref)
+    check_walk(b, out, ref)
+
+
 def test_all_particles_coincident():
     pm = np.zeros((100, 4), np.float32)
     pm[:, :3] = (1.0, 2.0, 3.0)

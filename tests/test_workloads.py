@@ -1,6 +1,7 @@
 """Pins for the seeded Plummer generator (paper_1204_2280_b200/workloads.py): closed forms of the
 Plummer model (P:L32 Results "Plummer spheres"; BASELINE.json configs: Henon units, 99.9 % mass cut)."""
 import numpy as np
+import pytest
 
 import oracle as O
 from paper_1204_2280_b200 import workloads as W
@@ -70,3 +71,21 @@ def test_no_duplicate_keys_at_config0():
     k = O.keys(pm, lo, side)
     big = (k[:, 0].astype(object) << 60) | (k[:, 1].astype(object) << 30) | k[:, 2].astype(object)
     assert len(set(big.tolist())) == 1 << 15
+
+
+def test_merger_workload_structure():
+    pm, vel = W.merger(40000)
+    m = pm[:, 3].astype(np.float64)
+    assert m.sum() == pytest.approx(1.0, rel=1e-6)
+    com = (m[:, None] * pm[:, :3]).sum(axis=0)
+    assert np.abs(com).max() < 0.02                                   # sampling noise of two finite spheres
+    mom = (m[:, None] * vel.astype(np.float64)).sum(axis=0)
+    assert np.abs(mom).max() < 0.01
+    a, b = pm[:30000], pm[30000:]
+    assert a[:, 0].mean() == pytest.approx(-1.5, abs=0.05) and b[:, 0].mean() == pytest.approx(4.5, abs=0.05)
+    ra = np.median(np.linalg.norm(a[:, :3] - a[:, :3].mean(axis=0), axis=1))
+    rb = np.median(np.linalg.norm(b[:, :3] - b[:, :3].mean(axis=0), axis=1))
+    assert rb / ra == pytest.approx(np.sqrt(1 / 3), rel=0.05)         # B is the smaller sphere
+    assert vel[:30000, 0].mean() > 0 > vel[30000:, 0].mean()          # approaching
+    pm2, _ = W.merger(40000)
+    assert np.array_equal(pm, pm2)                                    # seeded
