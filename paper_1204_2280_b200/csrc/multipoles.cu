@@ -153,43 +153,53 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         c_arrived[p] = 0;  // ready for the next step
         __threadfence();
         const uint32_t fc = t.first_child[p];
+        // ONE pass over the children (each record fetched once, two children's loads in flight per trip).  Moments
+        // are gathered about the first child's centre c0 -- at most a cell diagonal away from every other child, so
+        // the shift to the centre of mass below cancels at most one digit of the fp64 sums -- and moved to the COM at
+        // the end (parallel-axis theorem):
+        //   M = sum m_k,  S = sum m_k d_k,  T = sum (Q_k + m_k d_k d_k^T),  d_k = c_k - c0;
+        //   COM = c0 + S / M,  Q = T - M (S / M)(S / M)^T.
+        // A massless child has Q = 0 and m = 0 and drops out by itself.
         Mom q;
-        double sx = 0.0, sy = 0.0, sz = 0.0;
         float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
-        q.m = 0.0;
+        const double2* mo0 = reinterpret_cast<const double2*>(c_mom + (size_t)fc * 10);
+        double c0x = 0.0, c0y = 0.0, c0z = 0.0;
+        double M = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
+        double txx = 0.0, tyy = 0.0, tzz = 0.0, txy = 0.0, txz = 0.0, tyz = 0.0;
+#pragma unroll 2
         for (uint32_t k = 0; k < nc; ++k) {
-            const double2* mo = reinterpret_cast<const double2*>(c_mom + (size_t)(fc + k) * 10);
+            const double2 r0 = __ldcg(&mo0[5 * k + 0]), r1 = __ldcg(&mo0[5 * k + 1]), r2 = __ldcg(&mo0[5 * k + 2]),
+                          r3 = __ldcg(&mo0[5 * k + 3]), r4 = __ldcg(&mo0[5 * k + 4]);
             if (use_extent) {
                 const float2* bx = reinterpret_cast<const float2*>(c_box + (size_t)(fc + k) * 6);
                 const float2 b0 = __ldcg(&bx[0]), b1 = __ldcg(&bx[1]), b2 = __ldcg(&bx[2]);
                 mn[0] = fminf(mn[0], b0.x); mn[1] = fminf(mn[1], b0.y); mn[2] = fminf(mn[2], b1.x);
                 mx[0] = fmaxf(mx[0], b1.y); mx[1] = fmaxf(mx[1], b2.x); mx[2] = fmaxf(mx[2], b2.y);
             }
-            const double2 r0 = __ldcg(&mo[0]), r1 = __ldcg(&mo[1]);  // (m, cx), (cy, cz)
+            if (k == 0) { c0x = r0.y; c0y = r1.x; c0z = r1.y; }
             const double m = r0.x;
-            q.m += m;
-            sx += m * r0.y;
-            sy += m * r1.x;
-            sz += m * r1.y;
+            const double dx = r0.y - c0x, dy = r1.x - c0y, dz = r1.y - c0z;
+            M += m;
+            sx += m * dx; sy += m * dy; sz += m * dz;
+            txx += r2.x + m * dx * dx;
+            tyy += r2.y + m * dy * dy;
+            tzz += r3.x + m * dz * dz;
+            txy += r3.y + m * dx * dy;
+            txz += r4.x + m * dx * dz;
+            tyz += r4.y + m * dy * dz;
         }
+        q.m = M;
         q.cx = q.cy = q.cz = 0.0;
         q.xx = q.yy = q.zz = q.xy = q.xz = q.yz = 0.0;
-        if (q.m > 0.0) {
-            q.cx = sx / q.m; q.cy = sy / q.m; q.cz = sz / q.m;
-            for (uint32_t k = 0; k < nc; ++k) {
-                const double2* mo = reinterpret_cast<const double2*>(c_mom + (size_t)(fc + k) * 10);
-                const double2 r0 = __ldcg(&mo[0]), r1 = __ldcg(&mo[1]), r2 = __ldcg(&mo[2]), r3 = __ldcg(&mo[3]),
-                              r4 = __ldcg(&mo[4]);
-                const double m = r0.x;
-                if (!(m > 0.0)) continue;  // a massless child carries the geometric centre, not a COM
-                const double dx = r0.y - q.cx, dy = r1.x - q.cy, dz = r1.y - q.cz;
-                q.xx += r2.x + m * dx * dx;
-                q.yy += r2.y + m * dy * dy;
-                q.zz += r3.x + m * dz * dz;
-                q.xy += r3.y + m * dx * dy;
-                q.xz += r4.x + m * dx * dz;
-                q.yz += r4.y + m * dy * dz;
-            }
+        if (M > 0.0) {
+            const double ux = sx / M, uy = sy / M, uz = sz / M;
+            q.cx = c0x + ux; q.cy = c0y + uy; q.cz = c0z + uz;
+            q.xx = txx - M * ux * ux;
+            q.yy = tyy - M * uy * uy;
+            q.zz = tzz - M * uz * uz;
+            q.xy = txy - M * ux * uy;
+            q.xz = txz - M * ux * uz;
+            q.yz = tyz - M * uy * uz;
         }
         const uint32_t f = t.first[p];
         store_cell<use_extent>(q, mn, mx, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc,
