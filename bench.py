@@ -13,6 +13,11 @@ acc/pot inside the timed region).  The path does not shard (SURVEY.md section 8(
 --gpus N > 1 every rank runs the same step on its own replica, no collective on the data path, and `value` is
 the sum over ranks of N / (max over ranks of the time).
 
+The timed region (`value`, `ms_per_step`) runs the library UN-instrumented; the per-stage split (`stages`, and the
+walk time behind `roofline`) comes from a second set of K steps with the library's stage events switched on, and
+`instrumented_ms_per_step` says what that instrumentation costs.  `roofline.peak` is derived (SMs x 128 lanes x 2 flop
+x clocks.max.sm); `roofline.peak_measured` is bonsai_measure_fp32_peak() run in this process (FFMA2 and FFMA).
+
 --impl reference times the CPU oracle (oracle/, single thread, fp64), as it stands, on a bounded sample of the
 same workload; it needs no GPU.
 """
@@ -79,10 +84,40 @@ def oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, walk_budge
     return est, what
 
 
-def cpu_baseline(pm, theta, eps, ncrit, group_mode, group_cell, budget_s=15.0):
+def cpu_baseline(pm, theta, eps, ncrit, group_mode, group_cell, budget_s=12.0):
     est, what = oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, budget_s)
     return {"value": pm.shape[0] / est, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
             "est_full_step_s": est}
+
+
+def cpu_baseline_all_cores(pm, theta, eps, ncrit, group_mode, group_cell, budget_s=10.0):
+    """The same oracle with its walk under an outer parallel loop over groups (groups are independent) on every host
+    core -- SURVEY.md section 8(d) (ii); the paper's CPU side is a 4-core Xeon.  The stages before the
+    walk stay single-threaded as the oracle has them (~2 % of its time).  `cores` is read at run time."""
+    import oracle as O
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    t0 = time.perf_counter()
+    s = O.build(pm, 16, ncrit, group_mode, None, None, group_cell)
+    t_build = time.perf_counter() - t0
+    ng = s.groups.n_groups
+    probe = np.unique(np.linspace(0, ng - 1, min(ng, 16 * cores)).astype(np.uint32))
+    t0 = time.perf_counter()
+    O.walk_threads(theta, eps, s.sorted_pos_mass, s.tree, s.groups, probe, cores)
+    per_group = (time.perf_counter() - t0) / len(probe)
+    stride = 1
+    while per_group * ng / stride > budget_s and stride < ng:
+        stride *= 2
+    sel = np.arange(0, ng, stride, dtype=np.uint32)
+    t0 = time.perf_counter()
+    O.walk_threads(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, cores)
+    t_walk = time.perf_counter() - t0
+    n_sinks = int(s.groups.count[sel].sum())
+    est = t_build + t_walk * (s.groups.n_active / n_sinks)
+    what = (f"pre-walk stages single-threaded on all {pm.shape[0]} particles ({t_build:.2f} s) + walk of {len(sel)} of "
+            f"{ng} groups (every {stride}th, {n_sinks} sinks) on {cores} threads ({t_walk:.2f} s) scaled by "
+            f"{s.groups.n_active}/{n_sinks}")
+    return {"value": pm.shape[0] / est, "unit": UNIT, "cores": cores, "kind": "oracle, outer parallel loop over groups",
+            "sample": what, "est_full_step_s": est}
 
 
 def run_reference(args):
@@ -206,6 +241,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     from paper_1204_2280_b200 import Bonsai
+    from paper_1204_2280_b200.bonsai import measure_fp32_peak
     W, n, theta, eps = _workload(args.workload)
     pm = W.plummer(n)
     peaks = {}
@@ -217,7 +253,6 @@ def run_ours(args):
 
     stream = torch.cuda.Stream(dev)
     b = Bonsai(n, ncrit=args.ncrit, group_mode=args.group_mode, group_cell=args.group_cell, device=dev, stream=stream)
-    b.set_timing(True)
     d_pm = torch.from_numpy(pm).to(dev)
     d_out = torch.zeros((n, 4), dtype=torch.float32, device=dev)
     h_pm = torch.from_numpy(pm).pin_memory()
@@ -251,25 +286,36 @@ def run_ours(args):
         return e0, e1
 
     sampler = ClockSampler(local_rank) if rank == 0 else None   # started early: nvidia-smi takes a moment to come up
+    b.set_timing(False)
     for _ in range(args.warmup):
         one_step()
         b.sync()
-    # ---- timed region: exactly K steps, device-resident inputs ----
+    # ---- timed region: exactly K steps, device-resident inputs, library un-instrumented ----
     barrier()
     launches0 = b.launch_count()
     t_wall0 = time.perf_counter()
-    step_ms, stage_ms = [], []
+    step_ms = []
     for _ in range(args.steps):
         e0, e1 = one_step()
         b.sync()
         step_ms.append(e0.elapsed_time(e1))
-        stage_ms.append(b.stage_ms())
     barrier()
     t_wall1 = time.perf_counter()
     launches = b.launch_count() - launches0
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     sum_pp, sum_pc = b.interaction_totals()
     total_ms = float(sum(step_ms))
+
+    # ---- the same K steps with the library's stage events on: per-stage split, walk time of the roofline ----
+    b.set_timing(True)
+    one_step(); b.sync(); b.stage_ms()
+    inst_ms, stage_ms = [], []
+    for _ in range(args.steps):
+        e0, e1 = one_step()
+        b.sync()
+        inst_ms.append(e0.elapsed_time(e1))
+        stage_ms.append(b.stage_ms())
+    b.set_timing(False)
 
     # ---- end to end through the host-buffer call ----
     for _ in range(min(args.warmup, 2)):
@@ -296,37 +342,47 @@ def run_ours(args):
         n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
         peak_tf = n_sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
         achieved_tf = flop / (walk_ms * 1e-3) / 1e12
+        with torch.cuda.stream(stream):
+            peak_ffma2 = measure_fp32_peak(True, 40000, stream)
+            peak_ffma = measure_fp32_peak(False, 40000, stream)
+        peak_meas = max(peak_ffma2, peak_ffma)
         hbm = peaks.get("hbm_gbs", 6650.0)
         hbm_src = "measured" if "hbm_gbs" in peaks else "fallback"
-        # algorithmic bytes per particle of the HBM-bound stages
-        # keys: 16 in + 3 words out; sort: 6 pair passes over the mid and hi words x (8 in + 8 out), minus the index
-        # read of the first pass (iota) and the key write of the last; reorder: perm + record in, record + 3 key
-        # words out, plus the tie check re-reading the hi and mid words
-        alg_bytes = {"bbox": 16, "keys": 28, "sort": 6 * 16 - 8, "reorder": 48 + 8, "groups": 16 + 24 / args.ncrit}
         stages = {}
         for k, v in st.items():
             ent = {"ms": v, "share": v / sum(st.values())}
-            if k in alg_bytes and v > 0:
-                gbs = alg_bytes[k] * n / (v * 1e-3) / 1e9
-                ent.update({"alg_gbs": gbs, "hbm_frac": gbs / hbm})
+            if k in ALG_BYTES and v > 0:
+                gbs = ALG_BYTES[k](args) * n / (v * 1e-3) / 1e9
+                ent.update({"alg_bytes_per_particle": ALG_BYTES[k](args), "alg_gbs": gbs, "hbm_frac": gbs / hbm})
             stages[k] = ent
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": args.workload, "n": n, "theta": theta, "eps": eps, "nleaf": 16,
-                       "ncrit": args.ncrit, "group_mode": args.group_mode, "group_cell": args.group_cell, "parallelism": "replicas only",
-                       "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB fill, outside the event pair)",
-                       "paper_context": "GTX480: > 2.8e6 particles/s (PAPER.md:14), other hardware"},
+                       "ncrit": args.ncrit, "group_mode": args.group_mode, "group_cell": args.group_cell},
+            "notes": {"parallelism": "replicas only (no data-path collective)",
+                      "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB fill, outside the event pair)",
+                      "paper_context": "GTX480: > 2.8e6 particles/s (PAPER.md:14), other hardware",
+                      "groups": "group_mode 2 = runs of 64 sorted particles inside cells of <= group_cell particles: "
+                                "full lanes, but more interactions than tree-cell groups (group_mode 0), whose "
+                                "survey figure is 88.2 kflop per particle (SURVEY.md 8(d)) against "
+                                "roofline.flop_per_particle here; particles/s is the metric, the trade was measured"},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_total_ms / args.steps,
                     "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n},
             "gpu_launches": int(launches),
+            "instrumented_ms_per_step": float(np.mean(inst_ms)),
             "roofline": {"kernel": "k_walk", "bound": "alu", "achieved": achieved_tf, "peak": peak_tf,
-                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": walk_traffic(args),
+                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+                         "peak_measured": peak_meas, "frac_of_measured": achieved_tf / peak_meas,
+                         "peak_measured_source": f"bonsai_measure_fp32_peak in this process: FFMA2 {peak_ffma2:.2f}, "
+                                                 f"FFMA {peak_ffma:.2f} TFLOP/s (64 warps/SM, 8 chains, best of 3)",
+                         "traffic": walk_traffic(args),
                          "peak_source": f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x "
                                         f"{sm_max:.0f} MHz (clocks.max.sm); no fp32 entry in MEASURED_PEAKS.json",
                          "flop_convention": "20 per p-p, 63 per p-c (FMA = 2, rsqrt = 1)",
+                         "flop_per_particle": flop / n, "flop_per_particle_tree_cell_groups_survey": 88.2e3,
                          "walk_ms": walk_ms, "walk_share_of_step": walk_ms / sum(st.values()),
                          "interactions_per_s": (sum_pp + sum_pc) / (walk_ms * 1e-3),
                          "pp_per_particle": sum_pp / n, "pc_per_particle": sum_pc / n,
@@ -335,6 +391,8 @@ def run_ours(args):
         }
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell)
+            line["cpu_baseline_all_cores"] = cpu_baseline_all_cores(pm, theta, eps, args.ncrit, args.group_mode,
+                                                                    args.group_cell)
         print(json.dumps(line), flush=True)
     b.close()
     if world > 1:
@@ -343,13 +401,36 @@ def run_ours(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of k_walk from one `ncu --set full` capture of the default workload
-# (profiles/r1e_walk_ncu.md: 441.7 MB + 262.9 MB per launch); any other configuration has no capture.
-WALK_DRAM_BYTES_NCU = {("plummer_4m", 64, 2, 1024): 704.7e6}
+# Algorithmic bytes per particle of the HBM-bound stages (SURVEY.md section 8(d) floors):
+#   keys: 16 in + 3 key words out; sort: 6 pair passes over the mid and hi words x (8 in + 8 out), minus the index
+#   read of the first pass (iota) and the key write of the last; reorder: perm + record in, record + 3 key words out,
+#   plus the tie check re-reading the hi and mid words; build: the single-pass floor, 12 (keys once) + 4 (cell
+#   records, 0.23 cells x 16 B); groups: positions once + one box per group; multipoles: positions once + 0.23 cells
+#   x 48 B out + the children's records re-read by the internal cells (~0.05 x 48 B) = 30.
+ALG_BYTES = {
+    "bbox": lambda a: 16, "keys": lambda a: 28, "sort": lambda a: 6 * 16 - 8, "reorder": lambda a: 48 + 8,
+    "build": lambda a: 16, "groups": lambda a: 16 + 24 / a.ncrit, "multipoles": lambda a: 30,
+}
 
 
 def walk_traffic(args):
-    return WALK_DRAM_BYTES_NCU.get((args.workload, args.ncrit, args.group_mode, args.group_cell))
+    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of one k_walk launch, from the committed `ncu
+    --set full` capture profiles/walk_traffic.json -- valid only for the kernel it was taken from, so it is keyed by
+    the SHA-256 of the walk's sources and by the workload; anything else reports null (never a stale number)."""
+    import hashlib
+    try:
+        with open(os.path.join(ROOT, "profiles", "walk_traffic.json")) as f:
+            cap = json.load(f)
+        h = hashlib.sha256()
+        for rel in cap["sources"]:
+            with open(os.path.join(ROOT, rel), "rb") as f:
+                h.update(f.read())
+    except (OSError, KeyError, ValueError):
+        return None
+    key = [args.workload, args.ncrit, args.group_mode, args.group_cell]
+    if h.hexdigest() != cap.get("sources_sha256") or key != cap.get("config"):
+        return None
+    return cap["dram_bytes_read"] + cap["dram_bytes_write"]
 
 
 def main():

@@ -7,9 +7,11 @@
  * ('moving')", "construction of the tree-datastructure", "computation of the multipole
  * moments", "tree-traverse") map onto the calls below.  "All parts of the algorithm are
  * executed on the GPU" (Abstract): every pointer documented "device" below is a
- * CUDA device pointer, the host only sequences stages, and no call copies particle data
- * between host and device.  The paper states no formula or constant; the exact
- * arithmetic of every stage is the set of readings R1..R21 in DESIGN.md.
+ * CUDA device pointer and the host only sequences stages.  No call copies particle data
+ * between host and device, with ONE exception that exists for end-to-end measurement and
+ * for callers without device buffers: bonsai_step_host() (host pointers in and out, copies
+ * inside).  The paper states no formula or constant; the exact arithmetic of every stage
+ * is the set of readings R1..R31 in DESIGN.md.
  *
  * Conventions
  *   - All calls return an int: 0 (BONSAI_OK) or a negative BONSAI_E* code.  No exceptions, no
@@ -41,6 +43,8 @@ extern "C" {
 #define BONSAI_ECUDA      (-4)  /* a CUDA runtime call failed                                             */
 #define BONSAI_ENOMEM     (-5)  /* workspace smaller than bonsai_workspace_bytes()                        */
 
+#define BONSAI_THETA_MAX   1.15f /* R9/R11: largest opening angle accepted; below 2/sqrt(3) a sink's own leaf is
+                                    always opened, which the arithmetic removal of the self term relies on      */
 #define BONSAI_MAX_LEVEL   30   /* R1: 30 bits per axis, 90-bit Morton key (BASELINE.json north_star)     */
 #define BONSAI_N_STAGES    9
 
@@ -95,7 +99,8 @@ int bonsai_compute_multipoles(bonsai_ctx* ctx);
  * criterion  d2 > (l / theta + delta)^2  evaluated in fp32 exactly as R9 orders it (d = distance from the group's
  * box to the cell's COM); accepted cells act on every particle of the group as monopole + quadrupole
  * (particle-cell), rejected leaves particle by particle, with Plummer softening eps in every power of r (R10).
- *   theta >= 0 (0 = open everything = direct summation through the tree), eps >= 0, both finite
+ *   0 <= theta <= BONSAI_THETA_MAX (0 = open everything = direct summation through the tree; above 2/sqrt(3) a
+ *   cell containing a sink could be accepted, see R9), eps >= 0 and finite
  *   active_mask_dev  device u8[n] in LOAD order, or NULL = all particles are sinks.  A non-NULL mask rebuilds
  *                    the group list over the active particles for this call (R13, R19); all particles stay
  *                    sources.  Must stay valid until the call completed on the stream.
@@ -116,7 +121,9 @@ int bonsai_step_host(bonsai_ctx* ctx, const float* pos_mass_host, uint32_t n, fl
 /* Release the context (host memory only; the workspace belongs to the caller).  NULL is allowed. */
 void bonsai_destroy(bonsai_ctx* ctx);
 
-/* Wait for the stream and return the sticky device status (OK / ECAPACITY) or ECUDA. */
+/* Wait for the stream and return the sticky device status (OK / ECAPACITY) or ECUDA.  The status covers the work
+ * enqueued since the last bonsai_build_tree(): that call clears it (and repairs the internal counters an overflow
+ * leaves behind), so one failed step does not poison the context. */
 int bonsai_sync(bonsai_ctx* ctx);
 
 /* ---- introspection (parity tests and reporting).  All pointers returned are DEVICE pointers. ---- */
@@ -251,15 +258,22 @@ int bonsai_block_tick(bonsai_ctx* ctx, float* pos_mass_dev, float* vel_dev, floa
                       uint32_t n, uint64_t tick, float theta, float eps, float eta, float dt_max, uint32_t kmax,
                       int rebuild);
 
-/* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events between stages from then on;
- * bonsai_get_stage_ms() waits for the stream and writes milliseconds of the most recent execution of each
- * stage: 0 bbox, 1 keys, 2 sort, 3 reorder, 4 build, 5 groups, 6 multipoles, 7 walk, 8 integrate (the most
- * recent kick / drift / kick+drift launch). */
+/* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events around every stage from then on;
+ * bonsai_get_stage_ms() waits for the stream and writes, per stage, the milliseconds SUMMED over its executions
+ * since the previous bonsai_get_stage_ms() (or bonsai_set_timing) call -- up to 8 executions per stage:
+ * 0 bbox, 1 keys, 2 sort, 3 reorder, 4 build, 5 groups, 6 multipoles, 7 walk, 8 integrate (kicks, drifts). */
 int bonsai_set_timing(bonsai_ctx* ctx, int enable);
 int bonsai_get_stage_ms(bonsai_ctx* ctx, float out_ms[BONSAI_N_STAGES]);
 
 /* Number of kernel launches the library has enqueued since bonsai_create(). */
 uint64_t bonsai_get_launch_count(bonsai_ctx* ctx);
+
+/* Measurement support (not a step of the method): the FP32 throughput of the current CUDA device, measured with a
+ * register-only loop of independent chains of the instruction the walk's interaction loops are made of --
+ * packed != 0: fma.rn.f32x2 (SASS FFMA2), packed == 0: scalar FFMA -- `iters` rounds per thread, 64 warps per SM,
+ * best of three timed launches on `cuda_stream` (CUDA events).  Writes TFLOP/s (FMA = 2 flop) to *tflops_out.
+ * Blocks until done.  bench.py reports the walk's flop/s against this next to the derived peak.  EINVAL / ECUDA. */
+int bonsai_measure_fp32_peak(void* cuda_stream, int packed, int iters, double* tflops_out);
 
 const char* bonsai_strerror(int code);
 

@@ -186,6 +186,47 @@ def walk(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel=None):
     return WalkResult(acc, pot, n_pp, n_pc, nt[:n_sel], bl[:n_sel], sel_arr)
 
 
+def walk_threads(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel, threads):
+    """The same oracle_walk over the groups `sel`, split into `threads` interleaved subsets walked concurrently by
+    host threads (groups are independent and write disjoint rows; ctypes releases the GIL during the call).  This is
+    the "outer parallel loop over groups" of the all-cores CPU baseline (bench.py); no arithmetic lives here.
+    Returns the same WalkResult as walk(); g_ntests / g_borderline follow the order of `sel`."""
+    import threading
+    spm = _f32(sorted_pos_mass)
+    n = spm.shape[0]
+    sel = np.ascontiguousarray(sel, dtype=np.uint32)
+    acc = np.full((n, 3), np.nan, np.float64)
+    pot = np.full(n, np.nan, np.float64)
+    n_pp = np.zeros(n, np.uint32)
+    n_pc = np.zeros(n, np.uint32)
+    parts = [np.ascontiguousarray(sel[k::threads]) for k in range(threads)]
+    nts = [np.zeros(max(len(p), 1), np.uint32) for p in parts]
+    bls = [np.zeros(max(len(p), 1), np.uint8) for p in parts]
+    L = lib()
+
+    def work(k):
+        if len(parts[k]) == 0:
+            return
+        L.oracle_walk(C.c_float(theta), C.c_float(eps), _p(spm, C.c_float), C.c_uint32(n),
+                      _p(t.first, C.c_uint32), _p(t.count, C.c_uint32), _p(t.first_child, C.c_uint32),
+                      _p(t.n_child, C.c_uint32), _p(t.com_m, C.c_float), _p(t.quad, C.c_float),
+                      _p(t.delta, C.c_float), _p(t.lside, C.c_float), _p(g.active_list, C.c_uint32),
+                      _p(g.first, C.c_uint32), _p(g.count, C.c_uint32), _p(g.bmin, C.c_float),
+                      _p(g.bmax, C.c_float), C.c_uint32(len(parts[k])), _p(parts[k], C.c_uint32),
+                      _p(acc, C.c_double), _p(pot, C.c_double), _p(n_pp, C.c_uint32), _p(n_pc, C.c_uint32),
+                      _p(nts[k], C.c_uint32), _p(bls[k], C.c_uint8))
+
+    ths = [threading.Thread(target=work, args=(k,)) for k in range(threads)]
+    [th.start() for th in ths]
+    [th.join() for th in ths]
+    nt = np.zeros(len(sel), np.uint32)
+    bl = np.zeros(len(sel), np.uint8)
+    for k in range(threads):
+        nt[k::threads] = nts[k][:len(parts[k])]
+        bl[k::threads] = bls[k][:len(parts[k])]
+    return WalkResult(acc, pot, n_pp, n_pc, nt, bl, sel)
+
+
 def walk_lists(theta, t: Tree, bmin, bmax, cap=None):
     cap = cap if cap is not None else t.n_cells
     pc = np.zeros(cap, np.uint32)

@@ -31,6 +31,7 @@ SYMBOLS = (
     "bonsai_get_launch_count", "bonsai_strerror",
     "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
     "bonsai_timestep_rungs", "bonsai_active_mask", "bonsai_kick_rungs", "bonsai_block_tick",
+    "bonsai_measure_fp32_peak",
 )
 
 
@@ -99,6 +100,7 @@ def lib() -> C.CDLL:
     L.bonsai_drift.argtypes = [vp, vp, vp, u32, f32]
     L.bonsai_leapfrog_step.argtypes = [vp, vp, vp, vp, u32, f32, f32, f32]
     L.bonsai_diagnostics.argtypes = [vp, vp, vp, vp, u32, vp]
+    L.bonsai_measure_fp32_peak.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
     L.bonsai_strerror.argtypes = [C.c_int]
     L.bonsai_strerror.restype = C.c_char_p
     for name in SYMBOLS:  # fail loudly on a stale or partial library
@@ -114,6 +116,16 @@ def strerror(code: int) -> str:
 def _check(code: int, what: str) -> None:
     if code != OK:
         raise BonsaiError(code, what)
+
+
+def measure_fp32_peak(packed: bool = True, iters: int = 20000, stream: "torch.cuda.Stream | None" = None) -> float:
+    """bonsai_measure_fp32_peak: measured FP32 TFLOP/s of the current device (FFMA2 when packed, else FFMA)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
+    out = C.c_double(0.0)
+    st = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+    _check(lib().bonsai_measure_fp32_peak(st, int(bool(packed)), int(iters), C.byref(out)), "bonsai_measure_fp32_peak")
+    return float(out.value)
 
 
 def workspace_bytes(n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
@@ -212,7 +224,8 @@ class Bonsai:
              out: torch.Tensor | None = None) -> torch.Tensor:
         """Returns acc_pot float32[n, 4] = (ax, ay, az, phi) in load order (device tensor)."""
         if out is None:
-            out = torch.zeros((self.n, 4), dtype=torch.float32, device=self.device)
+            with torch.cuda.stream(self.stream):  # zero-filled on the stream the walk runs on
+                out = torch.zeros((self.n, 4), dtype=torch.float32, device=self.device)
         assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.shape == (self.n, 4)
         mptr = None
         if active_mask is not None:

@@ -69,7 +69,7 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     }
     t.ghist = cv.take<uint32_t>((size_t)kSortPasses * kRadix);
     t.look = cv.take<unsigned long long>((size_t)kRadix * n_tiles);
-    t.bbox_partial = cv.take<float>(6 * 148 * 16);
+    t.bbox_partial = cv.take<float>(6 * kBboxMaxBlocks);
     t.sorted_pos = cv.take<float4>(n);
     t.lcp = cv.take<int8_t>((size_t)n + 1);
     t.leaf_level = cv.take<int8_t>((size_t)n + 1);
@@ -108,19 +108,31 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     return (cv.off + kAlign - 1) / kAlign * kAlign;
 }
 
+// One timed interval of a stage.  A stage may run several times between two bonsai_get_stage_ms() calls (the
+// groups in bonsai_build_tree and again in a masked bonsai_walk, the kicks of a tick): every run takes the next
+// event pair of the stage and bonsai_get_stage_ms() sums them; beyond kStageIntervals the last pair is re-used.
 struct StageTimer {
     Ctx* c;
-    int stage;
-    StageTimer(Ctx* c_, int s) : c(c_), stage(s) {
-        if (c->timing) cudaEventRecord(c->ev[stage][0], c->stream);
+    int stage, slot;
+    StageTimer(Ctx* c_, int s) : c(c_), stage(s), slot(0) {
+        if (c->timing) {
+            slot = c->ev_count[stage] < kStageIntervals ? c->ev_count[stage] : kStageIntervals - 1;
+            cudaEventRecord(c->ev[stage][slot][0], c->stream);
+        }
     }
     ~StageTimer() {
         if (c->timing) {
-            cudaEventRecord(c->ev[stage][1], c->stream);
-            c->ev_valid[stage] = true;
+            cudaEventRecord(c->ev[stage][slot][1], c->stream);
+            if (c->ev_count[stage] < kStageIntervals) c->ev_count[stage] += 1;
         }
     }
 };
+
+// R9 / R11: the walk removes the self term arithmetically, which requires every sink's own leaf to be opened.  A cell
+// that contains the sink has d <= |x - COM| <= (sqrt(3)/2) l + delta, so it is never accepted while
+// l / theta > (sqrt(3)/2) l, i.e. theta < 2 / sqrt(3) = 1.1547; the library accepts theta in [0, 1.15].
+constexpr float kThetaMax = BONSAI_THETA_MAX;
+inline bool theta_ok(float theta) { return theta >= 0.0f && theta <= kThetaMax; }
 
 #define BONSAI_TRY(expr)                                  \
     do {                                                  \
@@ -166,12 +178,19 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.timing = false;
     c.launches = 0;
     for (int s = 0; s < BONSAI_N_STAGES; ++s) {
-        c.ev_valid[s] = false;
-        c.ev[s][0] = c.ev[s][1] = nullptr;
+        c.ev_count[s] = 0;
+        for (int k = 0; k < kStageIntervals; ++k) c.ev[s][k][0] = c.ev[s][k][1] = nullptr;
     }
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&c.num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete h;
+        return BONSAI_ECUDA;
+    }
+    c.device = dev;
+    // kernel attributes and occupancy are per device: set for every context (idempotent), never behind a
+    // process-wide flag
+    if (walk_prepare(&c) != cudaSuccess || sort_prepare(&c) != cudaSuccess) {
         delete h;
         return BONSAI_ECUDA;
     }
@@ -202,6 +221,9 @@ int bonsai_build_tree(bonsai_ctx* h) {
     if (!h) return BONSAI_EINVAL;
     Ctx* c = &h->c;
     if (c->state < 1) return BONSAI_ESTATE;
+    // the sticky status reports the work since the last build: a capacity overflow of an earlier step (reported by
+    // the bonsai_sync of that step) must not poison this one
+    BONSAI_TRY(stage_recover(c));
     { StageTimer t(c, 0); BONSAI_TRY(stage_bbox(c)); }
     { StageTimer t(c, 1); BONSAI_TRY(stage_keys(c)); }
     { StageTimer t(c, 2); BONSAI_TRY(stage_sort(c)); }
@@ -241,7 +263,7 @@ int bonsai_compute_multipoles(bonsai_ctx* h) {
 int bonsai_walk(bonsai_ctx* h, float theta, float eps, const uint8_t* active_mask_dev, float* acc_pot_dev_out) {
     if (!h || !acc_pot_dev_out) return BONSAI_EINVAL;
     if ((reinterpret_cast<uintptr_t>(acc_pot_dev_out) % 16) != 0) return BONSAI_EINVAL;
-    if (!(theta >= 0.0f) || !(eps >= 0.0f) || std::isinf(theta) || std::isinf(eps)) return BONSAI_EINVAL;
+    if (!theta_ok(theta) || !(eps >= 0.0f) || std::isinf(eps)) return BONSAI_EINVAL;
     Ctx* c = &h->c;
     if (c->state < 3) return BONSAI_ESTATE;
     if (active_mask_dev != nullptr || !c->groups_all_active) {
@@ -258,6 +280,7 @@ int bonsai_step_host(bonsai_ctx* h, const float* pos_mass_host, uint32_t n, floa
     if (!h || !pos_mass_host || !acc_pot_host_out) return BONSAI_EINVAL;
     Ctx* c = &h->c;
     if (n == 0 || n > c->n_max) return BONSAI_EINVAL;
+    if (!theta_ok(theta) || !(eps >= 0.0f) || std::isinf(eps)) return BONSAI_EINVAL;
     Buffers& b = c->b;
     BONSAI_TRY(cudaMemcpyAsync(b.host_in, pos_mass_host, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
     if (active_mask_host) {
@@ -319,7 +342,7 @@ int bonsai_leapfrog_step(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, flo
     if (!h || !pos_mass_dev || !vel_dev || !acc_pot_dev) return BONSAI_EINVAL;
     if (!aligned16(pos_mass_dev) || !aligned16(vel_dev) || !aligned16(acc_pot_dev)) return BONSAI_EINVAL;
     if (n == 0 || n > h->c.n_max || !std::isfinite(dt)) return BONSAI_EINVAL;
-    if (!(theta >= 0.0f) || !(eps >= 0.0f) || std::isinf(theta) || std::isinf(eps)) return BONSAI_EINVAL;
+    if (!theta_ok(theta) || !(eps >= 0.0f) || std::isinf(eps)) return BONSAI_EINVAL;
     Ctx* c = &h->c;
     const float half = 0.5f * dt;  // exact
     {
@@ -377,7 +400,7 @@ int bonsai_block_tick(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, float*
     if (!h || !pos_mass_dev || !vel_dev || !acc_pot_dev || !rung_dev) return BONSAI_EINVAL;
     if (!aligned16(pos_mass_dev) || !aligned16(vel_dev) || !aligned16(acc_pot_dev)) return BONSAI_EINVAL;
     if (n == 0 || n > h->c.n_max || kmax > 30u) return BONSAI_EINVAL;
-    if (!(theta >= 0.0f) || std::isinf(theta) || !(eta > 0.0f) || !(eps > 0.0f) || !(dt_max > 0.0f) || std::isinf(eta) ||
+    if (!theta_ok(theta) || !(eta > 0.0f) || !(eps > 0.0f) || !(dt_max > 0.0f) || std::isinf(eta) ||
         std::isinf(eps) || std::isinf(dt_max))
         return BONSAI_EINVAL;
     Ctx* c = &h->c;
@@ -409,8 +432,9 @@ int bonsai_block_tick(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, float*
 void bonsai_destroy(bonsai_ctx* h) {
     if (!h) return;
     for (int s = 0; s < BONSAI_N_STAGES; ++s)
-        for (int k = 0; k < 2; ++k)
-            if (h->c.ev[s][k]) cudaEventDestroy(h->c.ev[s][k]);
+        for (int i = 0; i < kStageIntervals; ++i)
+            for (int k = 0; k < 2; ++k)
+                if (h->c.ev[s][i][k]) cudaEventDestroy(h->c.ev[s][i][k]);
     delete h;
 }
 
@@ -513,12 +537,14 @@ int bonsai_get_interaction_totals(bonsai_ctx* h, uint64_t* sum_pp, uint64_t* sum
 int bonsai_set_timing(bonsai_ctx* h, int enable) {
     if (!h) return BONSAI_EINVAL;
     Ctx& c = h->c;
-    if (enable && !c.ev[0][0]) {
+    if (enable && !c.ev[0][0][0]) {
         for (int s = 0; s < BONSAI_N_STAGES; ++s)
-            for (int k = 0; k < 2; ++k)
-                if (cudaEventCreate(&c.ev[s][k]) != cudaSuccess) return BONSAI_ECUDA;
+            for (int i = 0; i < kStageIntervals; ++i)
+                for (int k = 0; k < 2; ++k)
+                    if (cudaEventCreate(&c.ev[s][i][k]) != cudaSuccess) return BONSAI_ECUDA;
     }
     c.timing = enable != 0;
+    for (int s = 0; s < BONSAI_N_STAGES; ++s) c.ev_count[s] = 0;
     return BONSAI_OK;
 }
 
@@ -528,8 +554,12 @@ int bonsai_get_stage_ms(bonsai_ctx* h, float out_ms[BONSAI_N_STAGES]) {
     if (cudaStreamSynchronize(c.stream) != cudaSuccess) return BONSAI_ECUDA;
     for (int s = 0; s < BONSAI_N_STAGES; ++s) {
         out_ms[s] = 0.0f;
-        if (c.ev_valid[s] && cudaEventElapsedTime(&out_ms[s], c.ev[s][0], c.ev[s][1]) != cudaSuccess)
-            return BONSAI_ECUDA;
+        for (int i = 0; i < c.ev_count[s]; ++i) {
+            float ms = 0.0f;
+            if (cudaEventElapsedTime(&ms, c.ev[s][i][0], c.ev[s][i][1]) != cudaSuccess) return BONSAI_ECUDA;
+            out_ms[s] += ms;
+        }
+        c.ev_count[s] = 0;
     }
     return BONSAI_OK;
 }

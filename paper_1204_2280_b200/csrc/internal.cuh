@@ -31,12 +31,17 @@ constexpr int kTreeTile = kTreeThreads * kTreeItems;  // particles per block
 constexpr int kLevelSlots = 32;                       // levels 0..30, padded
 constexpr int kMaxNleaf = 64;
 
+constexpr int kBboxMaxBlocks = 2048;       // rows of bbox_partial; stage_bbox clamps its grid to this
+constexpr int kStageIntervals = 8;         // event pairs per stage: a stage that runs several times between two
+                                           // bonsai_get_stage_ms() calls (groups in build and in a masked walk, the
+                                           // kicks of a tick) is summed over its intervals
+
 // ---- diagnostics (integrate.cu) ----------------------------------------------------------------
 constexpr int kDiagMaxBlocks = 1184;       // 8 blocks per SM on 148 SMs
 
 // ---- walk geometry (walk.cu) -------------------------------------------------------------------
 constexpr int kWalkWarps = 8;              // warps per block, one group per warp at a time
-constexpr int kWalkStack = 512;            // traversal stack entries per warp (see walk.cu for the bound)
+constexpr int kWalkStack = 512;            // traversal stack entries (runs of siblings) per warp; bound derived in walk.cu
 constexpr int kMaxNcrit = 64;
 
 // Device-resident control block at the start of the workspace (zeroed by bonsai_create).
@@ -55,7 +60,8 @@ struct Control {
     uint32_t sort_ticket;      // tile scheduler of k_sort_pass (reset by the tile that draws the last ticket)
     uint32_t diag_ticket;      // last-block-done counter of k_diagnostics
     uint32_t sort_fallback;    // set by k_sort_ties when a run of equal (hi, mid) is too long: the guarded chain runs
-    uint32_t pad1[3];
+    uint32_t recover_ticket;   // last-block-done counter of k_recover
+    uint32_t pad1[2];
     uint32_t level_offsets[32];  // first cell of level L; [31] = n_cells
     unsigned long long sum_pp;   // interaction totals of the last walk (sink-source pairs)
     unsigned long long sum_pc;
@@ -136,10 +142,12 @@ struct Ctx {
     uint32_t tree_n;           // particle count of the tree on the device (0 = none): bonsai_refresh_tree may reuse it
     bool tree_refreshed;       // positions were re-gathered into a frozen tree: multipoles take l from the extents (R25)
     bool timing;
-    cudaEvent_t ev[BONSAI_N_STAGES][2];
-    bool ev_valid[BONSAI_N_STAGES];
+    cudaEvent_t ev[BONSAI_N_STAGES][kStageIntervals][2];
+    int ev_count[BONSAI_N_STAGES];  // intervals recorded since the last bonsai_get_stage_ms()
     uint64_t launches;
     int num_sms;
+    int device;                // the CUDA device the context was created on
+    int walk_blocks_per_sm[4]; // occupancy of the four k_walk instances on this device (set in bonsai_create)
 };
 
 inline uint32_t div_up(uint32_t a, uint32_t b) { return (a + b - 1) / b; }
@@ -155,6 +163,9 @@ cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order);
 cudaError_t stage_multipoles(Ctx* c);
 cudaError_t cells_qraw(Ctx* c);  // fills c_qraw from c_mom (introspection)
 cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out);
+cudaError_t walk_prepare(Ctx* c);  // per-device kernel attributes and occupancy (bonsai_create)
+cudaError_t sort_prepare(Ctx* c);
+cudaError_t stage_recover(Ctx* c); // guarded: re-zeroes the arrival counters after a capacity overflow, clears the status
 size_t walk_smem_bytes(uint32_t nleaf);
 cudaError_t stage_kick(Ctx* c, float4* vel, const float4* acc, uint32_t n, float h, const uint8_t* mask);
 cudaError_t stage_drift(Ctx* c, float4* pos, const float4* vel, uint32_t n, float h);

@@ -223,6 +223,28 @@ cudaError_t cells_qraw(Ctx* c) {
     return cudaGetLastError();
 }
 
+// Recovery after a capacity overflow (guarded: returns at once when the device status is clear).  An overflow of the
+// cell arrays leaves arrival counters of cells whose children were cut off non-zero, which would corrupt every
+// later multipole pass of this context; the counters are re-zeroed and the sticky status is cleared by the last
+// block to finish, so that the status read by bonsai_sync() covers the work since the last bonsai_build_tree().
+__global__ void __launch_bounds__(256) k_recover(Control* __restrict__ ctl, uint32_t cap_cells,
+                                                 uint32_t* __restrict__ c_arrived) {
+    if (ctl->status == 0) return;  // the same answer in every block: only the last block to finish clears it
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < cap_cells; c += gridDim.x * blockDim.x) c_arrived[c] = 0;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0 && atomicAdd(&ctl->recover_ticket, 1u) == gridDim.x - 1) {
+        ctl->recover_ticket = 0;
+        ctl->status = 0;
+    }
+}
+
+cudaError_t stage_recover(Ctx* c) {
+    k_recover<<<c->num_sms * 2, 256, 0, c->stream>>>(c->b.ctl, c->cap_cells, c->b.c_arrived);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
 cudaError_t stage_multipoles(Ctx* c) {
     Buffers& b = c->b;
     const int s = c->sorted_buf;

@@ -467,7 +467,7 @@ __global__ void __launch_bounds__(256) k_reorder(const float4* __restrict__ pos,
 
 // ------------------------------------------------------------------------------------------------
 cudaError_t stage_bbox(Ctx* c) {
-    uint32_t blocks = min(div_up(c->n, 256 * 8), (uint32_t)(c->num_sms * 8));
+    uint32_t blocks = min(min(div_up(c->n, 256 * 8), (uint32_t)(c->num_sms * 8)), (uint32_t)kBboxMaxBlocks);
     k_bbox<<<blocks, 256, 0, c->stream>>>(c->pos_mass, c->n, c->b.bbox_partial, c->b.ctl);
     c->launches += 1;
     return cudaGetLastError();
@@ -549,19 +549,15 @@ __global__ void __launch_bounds__(256) k_sort_ties(const uint32_t* __restrict__ 
     }
 }
 
-static cudaError_t sort_prepare(Ctx* c, size_t* smem_out) {
-    static bool attr_set = false;
-    const size_t smem = sizeof(uint32_t) * ((kSortThreads / 32) * kRadix + 2 * kRadix);
-    *smem_out = smem;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_sort_pass<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_pass<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_pass<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+constexpr size_t kSortSmem = sizeof(uint32_t) * ((kSortThreads / 32) * kRadix + 2 * kRadix);
+
+// per device, at context creation (see walk_prepare)
+cudaError_t sort_prepare(Ctx* c) {
     (void)c;
-    return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(k_sort_pass<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_pass<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_pass<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSortSmem);
+    return e;
 }
 
 // Passes first_pass .. 8 of the LSD sort (pass p: word 2 - p / 3 = lo, mid, hi; digit p % 3), starting from the
@@ -569,9 +565,8 @@ static cudaError_t sort_prepare(Ctx* c, size_t* smem_out) {
 // by the callers below both chains leave the permutation in idx[0].
 static cudaError_t sort_chain(Ctx* c, int first_pass, int first_out, const uint32_t* guard) {
     Buffers& b = c->b;
-    size_t smem;
-    cudaError_t e = sort_prepare(c, &smem);
-    if (e != cudaSuccess) return e;
+    const size_t smem = kSortSmem;
+    cudaError_t e = cudaSuccess;
     SortPass a;
     a.n = c->n;
     a.n_tiles = div_up(c->n, kSortTile);

@@ -252,7 +252,15 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
     }
 }
 
-// Walk one chunk (<= 32 NS sinks) of group g.  Returns false on stack overflow.
+// Size of the traversal stack (kWalkStack runs of siblings per warp).  A round pops runs from the top until 32 cells
+// are gathered and pushes at most one run per tested cell, all one level below their parents.  New level-L runs
+// appear only when level-(L-1) cells are tested, and those lie BELOW every level-L run still on the stack, so a
+// round that reaches them has first consumed the level-L runs above: at any time at most 32 runs of one level are
+// stacked, and the stack never holds more than 32 x (levels that branch) entries.  A Plummer sphere of 2^22 particles
+// is 13 levels deep (32 x 13 = 416); single-child chains (coincident or very close particles) add one run per
+// level.  512 entries therefore cover every tree whose opened frontier branches over <= 16 levels; the theoretical
+// maximum of 30 levels (960) would cost twice the shared memory for trees that do not occur in practice, and is
+// not silently wrong either: an overflow stops the group and sets the sticky BONSAI_ECAPACITY status.
 __device__ __forceinline__ void team_barrier(int team, int warps) {
     asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "r"(warps * 32) : "memory");
 }
@@ -507,10 +515,10 @@ __global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
         const uint32_t warps = gridDim.x * kWalkWarps;
         int tsize = 1;
         float best = 3.0e38f;
-        for (int S = 1; S <= kWalkWarps; S *= 2) {
-            const float rounds = (float)(((unsigned long long)n_groups * S + warps - 1) / warps);
-            const float cost = rounds * (0.15f + 0.85f / (float)S);
-            if (cost < 0.95f * best) { best = cost; tsize = S; }
+        for (int ts = 1; ts <= kWalkWarps; ts *= 2) {
+            const float rounds = (float)(((unsigned long long)n_groups * ts + warps - 1) / warps);
+            const float cost = rounds * (0.15f + 0.85f / (float)ts);
+            if (cost < 0.95f * best) { best = cost; tsize = ts; }
         }
         if (tsize > 1) {
             walk_groups<kZeroEps, true>(S, a, n_groups, lane, w, tsize, s_team_g);
@@ -518,6 +526,22 @@ __global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
         }
     }
     walk_groups<kZeroEps, false>(S, a, n_groups, lane, w, 1, s_team_g);
+}
+
+using WalkKernel = void (*)(WalkArgs);
+static const WalkKernel kWalkKernels[4] = {k_walk<false, false>, k_walk<true, false>, k_walk<false, true>, k_walk<true, true>};
+
+// Kernel attributes are per device (and cheap to set again): done for every context at creation, so a second
+// device or a second host thread in the same process never launches without the dynamic shared memory opt-in.
+cudaError_t walk_prepare(Ctx* c) {
+    const size_t smem = walk_smem_bytes(c->prm.nleaf);
+    cudaError_t e;
+    for (int k = 0; k < 4; ++k) {
+        if ((e = cudaFuncSetAttribute(kWalkKernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->walk_blocks_per_sm[k], kWalkKernels[k], kWalkWarps * 32, smem)) != cudaSuccess) return e;
+        if (c->walk_blocks_per_sm[k] < 1) c->walk_blocks_per_sm[k] = 1;
+    }
+    return cudaSuccess;
 }
 
 cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
@@ -539,28 +563,17 @@ cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
     a.n_pp = b.n_pp;
     a.n_pc = b.n_pc;
     const size_t smem = walk_smem_bytes(c->prm.nleaf);
-    static bool attr_set = false;
-    static int blocks_per_sm[4] = {1, 1, 1, 1};
-    using Kernel = void (*)(WalkArgs);
-    static const Kernel kernels[4] = {k_walk<false, false>, k_walk<true, false>, k_walk<false, true>, k_walk<true, true>};
     cudaError_t e;
-    if (!attr_set) {
-        for (int k = 0; k < 4; ++k) {
-            if ((e = cudaFuncSetAttribute(kernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-            if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm[k], kernels[k], kWalkWarps * 32, smem)) != cudaSuccess) return e;
-        }
-        attr_set = true;
-    }
     // reset the ticket and the interaction totals (adjacent fields of the control block)
     if ((e = cudaMemsetAsync(&b.ctl->walk_ticket, 0, sizeof(uint32_t), c->stream)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(&b.ctl->sum_pp, 0, 2 * sizeof(unsigned long long), c->stream)) != cudaSuccess) return e;
     // a masked walk, or a small system, may have far fewer groups than resident warps: the team-capable kernel
     // adapts on the device; n / ncrit is a lower bound of the all-active group count known on the host
-    const unsigned long long resident_warps = (unsigned long long)c->num_sms * max(1, blocks_per_sm[2]) * kWalkWarps;
+    const unsigned long long resident_warps = (unsigned long long)c->num_sms * c->walk_blocks_per_sm[2] * kWalkWarps;
     const bool few_groups = !c->groups_all_active || 2ull * (c->n / c->prm.ncrit) <= resident_warps;
     const int which = ((a.eps2 == 0.0f) ? 1 : 0) + (few_groups ? 2 : 0);
-    const int grid = c->num_sms * max(1, blocks_per_sm[which]);
-    kernels[which]<<<grid, kWalkWarps * 32, smem, c->stream>>>(a);
+    const int grid = c->num_sms * c->walk_blocks_per_sm[which];
+    kWalkKernels[which]<<<grid, kWalkWarps * 32, smem, c->stream>>>(a);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -1,9 +1,9 @@
 """Parity of the block time-step calls (integrate.cu / bonsai_block_tick through the C-ABI binding) against the
 oracle (oracle/integrator_oracle.cpp R26-R27, oracle.block_tick).
 
-Gates: rungs, active masks and rung kicks BIT-EXACT; a run of block ticks (tree rebuilt, then refreshed) keeps the
-rung arrays identical to the oracle's and the trajectories within the walk's tolerance; one rung reproduces
-bonsai_leapfrog_step bit for bit."""
+Gates: rungs, active masks and rung kicks BIT-EXACT; a run of 8 block ticks (tree rebuilt, then refreshed), the two
+sides running independently from the same initial state, ends with rung arrays that differ for < 1 % of the
+particles and trajectories within the walk's tolerance; one rung reproduces bonsai_leapfrog_step bit for bit."""
 import numpy as np
 import pytest
 
@@ -78,8 +78,12 @@ def test_block_ticks_follow_the_oracle(rebuild_every):
     p, v = pm.copy(), O._vel4(vel)
     ap = O.force_f32(p, theta, eps)
     r = O.rungs(ap, eta, eps, dt_max, kmax)
-    assert np.array_equal(r_d.cpu().numpy(), r) or (r_d.cpu().numpy() != r).mean() < 1e-3
-    r = r_d.cpu().numpy().copy()                          # start both sides from the same rungs
+    flips0 = float((r_d.cpu().numpy() != r).mean())
+    assert flips0 < 1e-3                                  # |a| on a rung boundary within the walk's tolerance
+    # From here on the two sides run INDEPENDENTLY (nothing of the GPU's state is copied into the oracle's): a particle
+    # whose rung flipped on one side steps with a different dt from then on, so divergence accumulates over the 8
+    # ticks and is bounded at the end -- rung arrays differ for < 1 % of the particles, trajectories agree to the
+    # walk's tolerance for the bulk and to the size of one kick for the flipped few.
     prev = None
     walked = 0
     for tick in range(8):
@@ -88,18 +92,24 @@ def test_block_ticks_follow_the_oracle(rebuild_every):
         s, na = O.block_tick(p, v, ap, r, tick, theta, eps, eta, dt_max, kmax, prev=None if rebuild else prev)
         prev = s
         walked += na
-        # rungs flip only where |a| sits on a rung boundary within the walk's tolerance
-        assert (r_d.cpu().numpy() != r).mean() < 2e-3
-        r = r_d.cpu().numpy().copy()
     b.sync()
+    flips = float((r_d.cpu().numpy() != r).mean())
+    assert flips < 1e-2, flips
     assert walked < 0.7 * 8 * n                           # a real block scheme: not everybody every tick
     pg, vg = p_d.cpu().numpy(), v_d.cpu().numpy()
     assert np.array_equal(pg[:, 3], pm[:, 3])
-    dx = np.abs(pg[:, :3].astype(np.float64) - p[:, :3])
-    dv = np.abs(vg[:, :3].astype(np.float64) - v[:, :3])
+    dx = np.abs(pg[:, :3].astype(np.float64) - p[:, :3]).max(axis=1)
+    dv = np.abs(vg[:, :3].astype(np.float64) - v[:, :3]).max(axis=1)
     vrms = np.sqrt(np.mean(vel.astype(np.float64) ** 2))
-    assert np.median(dx) <= 2e-7 and np.quantile(dx, 0.999) <= 1e-5
-    assert np.median(dv) <= 1e-6 * vrms and np.quantile(dv, 0.999) <= 1e-3 * vrms
+    amax = np.abs(ap[:, :3]).max()
+    assert np.median(dx) <= 2e-7 and np.quantile(dx, 0.97) <= 1e-5
+    assert np.median(dv) <= 1e-6 * vrms and np.quantile(dv, 0.97) <= 1e-3 * vrms
+    # nobody is further off than a few kicks of the coarsest step
+    assert dv.max() <= 4 * amax * dt_max and dx.max() <= 4 * amax * dt_max * (8 * dt_max / 2 ** kmax) + 8 * dv.max() * dt_max
+    from test_gpu_parity import record
+    record("block_ticks", rebuild_every=rebuild_every, rung_flips_initial=flips0, rung_flips_after_8_ticks=flips,
+           dx_median=float(np.median(dx)), dx_q97=float(np.quantile(dx, 0.97)), dx_max=float(dx.max()),
+           dv_median_over_vrms=float(np.median(dv) / vrms), dv_max_over_vrms=float(dv.max() / vrms))
 
 
 def test_block_tick_errors():
