@@ -164,7 +164,7 @@ class WalkResult:
     sel: np.ndarray = field(default=None)
 
 
-def walk(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel=None):
+def walk(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel=None, order=2):
     spm = _f32(sorted_pos_mass)
     n = spm.shape[0]
     sel_arr = None if sel is None else np.ascontiguousarray(sel, dtype=np.uint32)
@@ -182,11 +182,11 @@ def walk(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel=None):
                       _p(g.first, C.c_uint32), _p(g.count, C.c_uint32), _p(g.bmin, C.c_float),
                       _p(g.bmax, C.c_float), C.c_uint32(n_sel), _p(sel_arr, C.c_uint32),
                       _p(acc, C.c_double), _p(pot, C.c_double), _p(n_pp, C.c_uint32), _p(n_pc, C.c_uint32),
-                      _p(nt, C.c_uint32), _p(bl, C.c_uint8))
+                      _p(nt, C.c_uint32), _p(bl, C.c_uint8), C.c_uint32(order))
     return WalkResult(acc, pot, n_pp, n_pc, nt[:n_sel], bl[:n_sel], sel_arr)
 
 
-def walk_threads(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel, threads):
+def walk_threads(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel, threads, order=2):
     """The same oracle_walk over the groups `sel`, split into `threads` interleaved subsets walked concurrently by
     host threads (groups are independent and write disjoint rows; ctypes releases the GIL during the call).  This is
     the "outer parallel loop over groups" of the all-cores CPU baseline (bench.py); no arithmetic lives here.
@@ -214,7 +214,7 @@ def walk_threads(theta, eps, sorted_pos_mass, t: Tree, g: Groups, sel, threads):
                       _p(g.first, C.c_uint32), _p(g.count, C.c_uint32), _p(g.bmin, C.c_float),
                       _p(g.bmax, C.c_float), C.c_uint32(len(parts[k])), _p(parts[k], C.c_uint32),
                       _p(acc, C.c_double), _p(pot, C.c_double), _p(n_pp, C.c_uint32), _p(n_pc, C.c_uint32),
-                      _p(nts[k], C.c_uint32), _p(bls[k], C.c_uint8))
+                      _p(nts[k], C.c_uint32), _p(bls[k], C.c_uint8), C.c_uint32(order))
 
     ths = [threading.Thread(target=work, args=(k,)) for k in range(threads)]
     [th.start() for th in ths]
@@ -272,8 +272,20 @@ class Step:
         return out
 
 
-def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cells=None, group_cell=1024) -> Step:
-    """O1..O6: box, keys, sort, reorder, tree, groups, multipoles.  active_mask is in LOAD order."""
+def tight_mac(sorted_pos_mass, t: Tree):
+    """R28 (oracle/mac_oracle.cpp): replace t.lside / t.delta by the side and COM offset of each cell's exact particle
+    box; returns the boxes float32[n_cells, 6] (bmin xyz, bmax xyz)."""
+    spm = _f32(sorted_pos_mass)
+    box = np.zeros((t.n_cells, 6), np.float32)
+    lib().oracle_tight_mac(_p(spm, C.c_float), C.c_uint32(t.n_cells), _p(t.first, C.c_uint32), _p(t.count, C.c_uint32),
+                           _p(t.lside, C.c_float), _p(t.delta, C.c_float), _p(box, C.c_float))
+    return box
+
+
+def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cells=None, group_cell=1024,
+          mac_mode=0) -> Step:
+    """O1..O6: box, keys, sort, reorder, tree, groups, multipoles.  active_mask is in LOAD order.
+    mac_mode = 1: the tight MAC of R28 (cell size and centre from the particle box)."""
     pm = _f32(pos_mass)
     lo, side = box(pm)
     k = keys(pm, lo, side)
@@ -283,13 +295,15 @@ def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cell
     act_sorted = None if active_mask is None else np.ascontiguousarray(active_mask, np.uint8)[perm]
     g = groups(group_mode, ncrit, spm, t, act_sorted, group_cell)
     multipoles(spm, sk, lo, side, t)
+    if mac_mode == 1:
+        tight_mac(spm, t)
     return Step(lo, side, k, perm, spm, sk, t, g)
 
 
 def full_step(pos_mass, theta, eps, nleaf=16, ncrit=64, group_mode=2, active_mask=None, sel=None,
-              group_cell=1024) -> Step:
-    s = build(pos_mass, nleaf, ncrit, group_mode, active_mask, None, group_cell)
-    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
+              group_cell=1024, mac_mode=0, order=2) -> Step:
+    s = build(pos_mass, nleaf, ncrit, group_mode, active_mask, None, group_cell, mac_mode)
+    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, order)
     return s
 
 
@@ -359,7 +373,8 @@ def leapfrog(pos_mass, vel, theta, eps, dt, n_steps, acc_pot=None, **kw):
 
 # ---- row f1: refreshed tree (oracle/refresh_oracle.cpp, R25) --------------------------------
 
-def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, group_cell=1024) -> Step:
+def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, group_cell=1024,
+            mac_mode=0) -> Step:
     """The structures of ``prev`` (permutation, keys, cells, group membership) carried over to moved particles.
 
     pos_mass is the SAME particles in the SAME load order as the build that produced ``prev``.
@@ -372,6 +387,9 @@ def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=
     act_sorted = None if active_mask is None else np.ascontiguousarray(active_mask, np.uint8)[prev.perm]
     g = groups(group_mode, ncrit, spm, t, act_sorted, group_cell)
     multipoles(spm, prev.sorted_keys, prev.lo, prev.side, t)
+    if mac_mode == 1:  # R28: the particle boxes are recomputed from the new positions; nothing grows (R25 not needed)
+        tight_mac(spm, t)
+        return Step(prev.lo, prev.side, prev.keys, prev.perm, spm, prev.sorted_keys, t, g)
     lo = _f32(prev.lo)
     sk = np.ascontiguousarray(prev.sorted_keys, dtype=np.uint32)
     lib().oracle_extent_side(_p(spm, C.c_float), _p(sk, C.c_uint32), _p(lo, C.c_float), C.c_double(prev.side),
@@ -380,9 +398,9 @@ def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=
     return Step(prev.lo, prev.side, prev.keys, prev.perm, spm, prev.sorted_keys, t, g)
 
 
-def refreshed_step(prev: Step, pos_mass, theta, eps, sel=None, **kw) -> Step:
+def refreshed_step(prev: Step, pos_mass, theta, eps, sel=None, order=2, **kw) -> Step:
     s = refresh(prev, pos_mass, **kw)
-    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel)
+    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, order)
     return s
 
 

@@ -351,6 +351,7 @@ void oracle_multipoles(const float* sorted_pos_mass, const uint32_t* sorted_keys
 //        acc += dr (M r^-3 - 3/2 tr r^-5 + 15/2 q r^-7) - 3 r^-5 Qr
 // Outputs are indexed by SORTED particle index (only entries of walked particles are written):
 //   acc[3*i..], pot[i], n_pp[i] = (sum of leaf counts in G's p-p list) - 1, n_pc[i] = |p-c list|.
+// order = 1 (R29): a p-c term is  pot -= M r^-1;  acc += M r^-3 dr  only.
 // Per selected group k (position in sel): g_ntests[k] = number of MAC tests; g_borderline[k] = 1 if
 // any test had |d2 - rc2| <= 1e-5 rc2 (fp64 on the fp32 inputs).
 // -------------------------------------------------------------------------------------
@@ -360,7 +361,9 @@ void oracle_walk(float theta, float eps, const float* sorted_pos_mass, uint32_t 
                  const float* lside, const uint32_t* active_list, const uint32_t* gfirst,
                  const uint32_t* gcount, const float* gbmin, const float* gbmax, uint32_t n_sel,
                  const uint32_t* sel, double* acc, double* pot, uint32_t* n_pp, uint32_t* n_pc,
-                 uint32_t* g_ntests, uint8_t* g_borderline) {
+                 uint32_t* g_ntests, uint8_t* g_borderline, uint32_t order) {
+    // order: 1 = accepted cells act as monopoles only (R29, oracle/mac_oracle.cpp); anything else = monopole +
+    // quadrupole (R8, the default).
     (void)n;
     volatile float inv_theta_v = 1.0f / theta;
     const float inv_theta = inv_theta_v;
@@ -426,6 +429,14 @@ void oracle_walk(float theta, float eps, const float* sorted_pos_mass, uint32_t 
                 double dy = (double)com_m[4 * c + 1] - yi;
                 double dz = (double)com_m[4 * c + 2] - zi;
                 double M = com_m[4 * c + 3];
+                if (order == 1) {
+                    double r2 = dx * dx + dy * dy + dz * dz + e2;
+                    double rinv = 1.0 / std::sqrt(r2);
+                    double rinv3 = rinv * rinv * rinv;
+                    ph -= M * rinv;
+                    ax += M * rinv3 * dx; ay += M * rinv3 * dy; az += M * rinv3 * dz;
+                    continue;
+                }
                 double Qxx = quad[6 * c + 0], Qyy = quad[6 * c + 1], Qzz = quad[6 * c + 2];
                 double Qxy = quad[6 * c + 3], Qxz = quad[6 * c + 4], Qyz = quad[6 * c + 5];
                 double r2 = dx * dx + dy * dy + dz * dz + e2;

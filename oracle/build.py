@@ -10,7 +10,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRCS = [os.path.join(HERE, "bonsai_oracle.cpp"), os.path.join(HERE, "integrator_oracle.cpp"),
-        os.path.join(HERE, "refresh_oracle.cpp")]
+        os.path.join(HERE, "refresh_oracle.cpp"), os.path.join(HERE, "mac_oracle.cpp")]
 LIB = os.path.join(HERE, "liboracle.so")
 
 
