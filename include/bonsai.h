@@ -61,6 +61,11 @@ typedef struct {
     uint32_t group_cell; /* [1024] mode 2: a group never crosses the boundary of a cell holding more than
                             group_cell particles (the containers are the cells with count <= group_cell whose
                             parent has more); >= ncrit                                                        */
+    uint32_t mac_mode;   /* [0] size and centre of a cell in the opening test ("MAC"): 0 = geometric cell
+                            (side l = root side / 2^level, geometric centre; R9), 1 = tight: the exact bounding box
+                            of the cell's particles, l_t = its longest side, centre = its midpoint (R28)         */
+    uint32_t order;      /* [2] multipole order of a particle-cell interaction: 2 = monopole + quadrupole (R8),
+                            1 = monopole only (R29); 0 = default                                                */
 } bonsai_params;
 
 /* Bytes of device workspace bonsai_create() needs for up to n_max particles (0 on bad arguments). */

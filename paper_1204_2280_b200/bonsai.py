@@ -37,7 +37,8 @@ SYMBOLS = (
 
 class Params(C.Structure):
     _fields_ = [("nleaf", C.c_uint32), ("ncrit", C.c_uint32), ("group_mode", C.c_uint32),
-                ("cap_cells", C.c_uint32), ("group_cell", C.c_uint32)]
+                ("cap_cells", C.c_uint32), ("group_cell", C.c_uint32), ("mac_mode", C.c_uint32),
+                ("order", C.c_uint32)]
 
 
 class CellsView(C.Structure):
@@ -129,8 +130,8 @@ def measure_fp32_peak(packed: bool = True, iters: int = 20000, stream: "torch.cu
 
 
 def workspace_bytes(n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
-                    cap_cells: int = 0, group_cell: int = 0) -> int:
-    p = Params(nleaf, ncrit, group_mode, cap_cells, group_cell)
+                    cap_cells: int = 0, group_cell: int = 0, mac_mode: int = 0, order: int = 2) -> int:
+    p = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order)
     return int(lib().bonsai_workspace_bytes(n_max, C.byref(p)))
 
 
@@ -175,14 +176,14 @@ class Bonsai:
 
     def __init__(self, n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
                  cap_cells: int = 0, group_cell: int = 0, device: str | torch.device = "cuda:0",
-                 stream: "torch.cuda.Stream | None" = None):
+                 stream: "torch.cuda.Stream | None" = None, mac_mode: int = 0, order: int = 2):
         if not torch.cuda.is_available():
             raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
         self.device = torch.device(device)
         self._L = lib()
         self.n_max = int(n_max)
         self.n = 0
-        self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell)
+        self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order)
         nbytes = int(self._L.bonsai_workspace_bytes(self.n_max, C.byref(self.params)))
         if nbytes == 0:
             raise BonsaiError(EINVAL, "bonsai_workspace_bytes")

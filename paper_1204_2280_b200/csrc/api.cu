@@ -30,8 +30,10 @@ struct Carver {
 
 bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out) {
     bonsai_params p;
-    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0;
+    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0; p.mac_mode = 0; p.order = 2;
     if (in) {
+        p.mac_mode = in->mac_mode;
+        if (in->order) p.order = in->order;
         if (in->nleaf) p.nleaf = in->nleaf;
         if (in->ncrit) p.ncrit = in->ncrit;
         p.group_mode = in->group_mode;
@@ -49,6 +51,7 @@ bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out)
     if (p.nleaf < 1 || p.nleaf > (uint32_t)kMaxNleaf) return false;
     if (p.ncrit < 1 || p.ncrit > (uint32_t)kMaxNcrit) return false;
     if (p.group_mode > 2) return false;
+    if (p.mac_mode > 1 || p.order < 1 || p.order > 2) return false;
     if (p.cap_cells < 1 || p.cap_cells >= (1u << 29)) return false;  // walk stack entries pack the id into 29 bits
     *out = p;
     return true;

@@ -147,7 +147,7 @@ struct Ctx {
     uint64_t launches;
     int num_sms;
     int device;                // the CUDA device the context was created on
-    int walk_blocks_per_sm[4]; // occupancy of the four k_walk instances on this device (set in bonsai_create)
+    int walk_blocks_per_sm[8]; // occupancy of the k_walk instances on this device (set in bonsai_create)
 };
 
 inline uint32_t div_up(uint32_t a, uint32_t b) { return (a + b - 1) / b; }

@@ -30,7 +30,10 @@ struct Mom {
     double m, cx, cy, cz, xx, yy, zz, xy, xz, yz;
 };
 
-template <bool use_extent>
+// kBox: the exact fp32 bounding box of the cell's members is available (mn, mx) and is stored for the parent;
+// kTight: R28 -- the side and centre that enter the opening test are those of that box (mac_mode = 1); otherwise, with
+// kBox alone, R25 -- a refreshed tree lets the geometric side grow to contain the members.
+template <bool kBox, bool kTight>
 __device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], const float (&mx)[3],
                                            uint32_t c, int L, uint32_t khi, uint32_t kmid, uint32_t klo,
                                            const Control* __restrict__ ctl, uint32_t link_first, uint32_t link_info,
@@ -47,17 +50,27 @@ __device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], c
         const uint32_t ca = (L == 0) ? 0u : (qa >> (kMaxLevel - L));
         g[a] = __dadd_rn((double)ctl->lo[a], __dmul_rn(__dadd_rn((double)ca, 0.5), l));
     }
-    if (use_extent) {
-        float2* bx = reinterpret_cast<float2*>(c_box + (size_t)c * 6);  // only a refreshed tree needs the boxes
+    if (kBox) {
+        float2* bx = reinterpret_cast<float2*>(c_box + (size_t)c * 6);  // only refreshed trees and the tight MAC need the boxes
         __stcg(&bx[0], make_float2(mn[0], mn[1]));
         __stcg(&bx[1], make_float2(mn[2], mx[0]));
         __stcg(&bx[2], make_float2(mx[1], mx[2]));
         // R25 (refreshed tree): the side becomes the side of the smallest cube about the geometric centre that
         // holds every member, never less than the geometric side: l = max(l, 2 max_axis max(g - min, max - g)), fp64
-        double e = 0.0;
+        if (kTight) {
+            // R28: l_t = longest side of the particle box, centre = its midpoint (fp64 on the exact fp32 bounds)
+            l = 0.0;
 #pragma unroll
-        for (int d = 0; d < 3; ++d) e = fmax(e, fmax(__dadd_rn(g[d], -(double)mn[d]), __dadd_rn((double)mx[d], -g[d])));
-        l = fmax(l, __dmul_rn(2.0, e));
+            for (int d = 0; d < 3; ++d) {
+                l = fmax(l, __dadd_rn((double)mx[d], -(double)mn[d]));
+                g[d] = __dmul_rn(0.5, __dadd_rn((double)mn[d], (double)mx[d]));
+            }
+        } else {
+            double e = 0.0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) e = fmax(e, fmax(__dadd_rn(g[d], -(double)mn[d]), __dadd_rn((double)mx[d], -g[d])));
+            l = fmax(l, __dmul_rn(2.0, e));
+        }
     }
     Mom o = q;
     if (!(q.m > 0.0)) {  // only zero-mass members: COM is undefined, take the geometric centre (R8)
@@ -94,7 +107,7 @@ struct TreeView {
     const uint32_t *level, *first, *count, *first_child, *n_child, *parent;
 };
 
-template <bool use_extent>
+template <bool kBox, bool kTight>
 __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ ctl, uint32_t cap_cells, TreeView t,
                                                     const float4* __restrict__ sorted_pos,
                                                     const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
@@ -114,7 +127,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         for (uint32_t k = 0; k < cnt; ++k) {
             const float4 p = __ldg(&sorted_pos[f + k]);
             const double m = (double)p.w;
-            if (use_extent) {
+            if (kBox) {
                 mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
                 mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
                 mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
@@ -141,7 +154,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
                 q.yz = __dadd_rn(q.yz, __dmul_rn(__dmul_rn(m, dy), dz));
             }
         }
-        store_cell<use_extent>(q, mn, mx, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f,
+        store_cell<kBox, kTight>(q, mn, mx, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f,
                    kLeafBit | cnt, c_mom, c_box, c_mac, c_quad, c_qraw);
     }
     for (;;) {
@@ -170,7 +183,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         for (uint32_t k = 0; k < nc; ++k) {
             const double2 r0 = __ldcg(&mo0[5 * k + 0]), r1 = __ldcg(&mo0[5 * k + 1]), r2 = __ldcg(&mo0[5 * k + 2]),
                           r3 = __ldcg(&mo0[5 * k + 3]), r4 = __ldcg(&mo0[5 * k + 4]);
-            if (use_extent) {
+            if (kBox) {
                 const float2* bx = reinterpret_cast<const float2*>(c_box + (size_t)(fc + k) * 6);
                 const float2 b0 = __ldcg(&bx[0]), b1 = __ldcg(&bx[1]), b2 = __ldcg(&bx[2]);
                 mn[0] = fminf(mn[0], b0.x); mn[1] = fminf(mn[1], b0.y); mn[2] = fminf(mn[2], b1.x);
@@ -202,7 +215,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
             q.yz = tyz - M * uy * uz;
         }
         const uint32_t f = t.first[p];
-        store_cell<use_extent>(q, mn, mx, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc,
+        store_cell<kBox, kTight>(q, mn, mx, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc,
                    c_mom, c_box, c_mac, c_quad, c_qraw);
         c = p;
     }
@@ -250,14 +263,13 @@ cudaError_t stage_multipoles(Ctx* c) {
     const int s = c->sorted_buf;
     TreeView t{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
     const dim3 grid(div_up(c->cap_cells, 128));
-    if (c->tree_refreshed)
-        k_multipoles<true><<<grid, 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1],
-                                                        b.key[s][2], b.c_mom, b.c_mac, b.c_quad, b.c_qraw, b.c_box,
-                                                        b.c_arrived);
-    else
-        k_multipoles<false><<<grid, 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1],
-                                                         b.key[s][2], b.c_mom, b.c_mac, b.c_quad, b.c_qraw, b.c_box,
-                                                         b.c_arrived);
+    using Kernel = void (*)(const Control*, uint32_t, TreeView, const float4*, const uint32_t*, const uint32_t*, const uint32_t*,
+                            double*, CellMac*, CellQuad*, float*, float*, uint32_t*);
+    const Kernel k = (c->prm.mac_mode == 1) ? (Kernel)k_multipoles<true, true>
+                     : c->tree_refreshed    ? (Kernel)k_multipoles<true, false>
+                                            : (Kernel)k_multipoles<false, false>;
+    k<<<grid, 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1], b.key[s][2], b.c_mom,
+                                   b.c_mac, b.c_quad, b.c_qraw, b.c_box, b.c_arrived);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -267,7 +267,9 @@ __device__ __forceinline__ void team_barrier(int team, int warps) {
 
 // kTeam: this warp is member `slot` of a team of `tsize` warps (WarpSmem of member j = (&S)[j - slot]) that walks
 // the chunk together; see the header.  kTeam = false compiles to the single-warp walk.
-template <int NS, bool kZeroEps, bool kTeam>
+// kMono: R29 -- accepted cells act as monopoles only: (COM, M) is a point source like any particle, so it joins the
+// p-p ring and the p-c kernel is never called; lists and counts are those of the quadrupole walk.
+template <int NS, bool kZeroEps, bool kTeam, bool kMono>
 __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int lane, uint32_t sink_first, uint32_t ns,
                                            const float (&bmin)[3], const float (&bmax)[3], int team, int slot,
                                            int tsize) {
@@ -334,9 +336,10 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
         // ---- opening test (R9), every operation rounded once, in this order ----
         bool accept = false, leaf = false;
         uint32_t link_first = 0, info = 0;
+        float4 m0 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
         if (valid) {
             const float4* m = reinterpret_cast<const float4*>(a.mac + cell);
-            const float4 m0 = __ldg(m);
+            m0 = __ldg(m);
             const float4 m1 = __ldg(m + 1);
             const float dx = fmaxf(0.0f, fmaxf(__fsub_rn(bmin[0], m0.x), __fsub_rn(m0.x, bmax[0])));
             const float dy = fmaxf(0.0f, fmaxf(__fsub_rn(bmin[1], m0.y), __fsub_rn(m0.y, bmax[1])));
@@ -361,6 +364,21 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
         // ---- accepted cells ----
         const bool acc = valid && accept;
         const uint32_t am = __ballot_sync(0xFFFFFFFFu, acc);
+        if constexpr (kMono) {
+            if (am) {
+                if (acc) {
+                    const uint32_t slot_w = pp_w + __popc(am & lt);
+                    if (!kTeam || ((slot_w >> 5) & tmask) == uslot) S.pp[slot_w & 63u] = m0;  // (COM, M)
+                }
+                pp_w += __popc(am);
+                npc += __popc(am);
+                __syncwarp();
+                if (pp_w - pp_r >= 32u) {
+                    if (!kTeam || ((pp_r >> 5) & tmask) == uslot) eval_pp<NS, kZeroEps>(S, pp_r, 32, a.eps2, s);
+                    pp_r += 32u;
+                }
+            }
+        } else {
         if (acc) S.pc_ids[(pc_w + __popc(am & lt)) & 63u] = cell;
         pc_w += __popc(am);
         npc += __popc(am);
@@ -368,6 +386,7 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
         if (pc_w - pc_r >= 32u) {
             if (!kTeam || ((pc_r >> 5) & tmask) == uslot) eval_pc<NS>(S, a, pc_r, 32, lane, s);
             pc_r += 32u;
+        }
         }
         // ---- rejected leaves: expand into particles ----
         const bool oleaf = valid && !accept && leaf;
@@ -462,7 +481,7 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
     return true;
 }
 
-template <bool kZeroEps, bool kTeam>
+template <bool kZeroEps, bool kTeam, bool kMono>
 __device__ __forceinline__ void walk_groups(WarpSmem& S, const WalkArgs& a, uint32_t n_groups, int lane, int w, int tsize,
                                             uint32_t* s_team_g) {
     const int team = kTeam ? w / tsize : w, slot = kTeam ? w % tsize : 0;
@@ -490,8 +509,8 @@ __device__ __forceinline__ void walk_groups(WarpSmem& S, const WalkArgs& a, uint
         for (uint32_t c0 = 0; c0 < gc; c0 += 64u) {
             const uint32_t ns = min(64u, gc - c0);
             bool ok;
-            if (ns > 32u) ok = walk_chunk<2, kZeroEps, kTeam>(S, a, lane, gf + c0, ns, bmin, bmax, team, slot, tsize);
-            else ok = walk_chunk<1, kZeroEps, kTeam>(S, a, lane, gf + c0, ns, bmin, bmax, team, slot, tsize);
+            if (ns > 32u) ok = walk_chunk<2, kZeroEps, kTeam, kMono>(S, a, lane, gf + c0, ns, bmin, bmax, team, slot, tsize);
+            else ok = walk_chunk<1, kZeroEps, kTeam, kMono>(S, a, lane, gf + c0, ns, bmin, bmax, team, slot, tsize);
             if (!ok && lane == 0) a.ctl->status = BONSAI_ECAPACITY;
             __syncwarp();
         }
@@ -500,7 +519,7 @@ __device__ __forceinline__ void walk_groups(WarpSmem& S, const WalkArgs& a, uint
 
 // kTeams = false: the plain one-warp-per-group kernel (all particles active: always enough groups).
 // kTeams = true: launched for masked walks; picks the team size from the number of groups on the device.
-template <bool kZeroEps, bool kTeams>
+template <bool kZeroEps, bool kTeams, bool kMono>
 __global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_team_g[kWalkWarps];
@@ -521,22 +540,25 @@ __global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
             if (cost < 0.95f * best) { best = cost; tsize = ts; }
         }
         if (tsize > 1) {
-            walk_groups<kZeroEps, true>(S, a, n_groups, lane, w, tsize, s_team_g);
+            walk_groups<kZeroEps, true, kMono>(S, a, n_groups, lane, w, tsize, s_team_g);
             return;
         }
     }
-    walk_groups<kZeroEps, false>(S, a, n_groups, lane, w, 1, s_team_g);
+    walk_groups<kZeroEps, false, kMono>(S, a, n_groups, lane, w, 1, s_team_g);
 }
 
 using WalkKernel = void (*)(WalkArgs);
-static const WalkKernel kWalkKernels[4] = {k_walk<false, false>, k_walk<true, false>, k_walk<false, true>, k_walk<true, true>};
+// index = (eps == 0) + 2 (team-capable) + 4 (monopole only)
+static const WalkKernel kWalkKernels[8] = {k_walk<false, false, false>, k_walk<true, false, false>, k_walk<false, true, false>,
+                                           k_walk<true, true, false>,   k_walk<false, false, true>, k_walk<true, false, true>,
+                                           k_walk<false, true, true>,   k_walk<true, true, true>};
 
 // Kernel attributes are per device (and cheap to set again): done for every context at creation, so a second
 // device or a second host thread in the same process never launches without the dynamic shared memory opt-in.
 cudaError_t walk_prepare(Ctx* c) {
     const size_t smem = walk_smem_bytes(c->prm.nleaf);
     cudaError_t e;
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < 8; ++k) {
         if ((e = cudaFuncSetAttribute(kWalkKernels[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->walk_blocks_per_sm[k], kWalkKernels[k], kWalkWarps * 32, smem)) != cudaSuccess) return e;
         if (c->walk_blocks_per_sm[k] < 1) c->walk_blocks_per_sm[k] = 1;
@@ -571,7 +593,7 @@ cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
     // adapts on the device; n / ncrit is a lower bound of the all-active group count known on the host
     const unsigned long long resident_warps = (unsigned long long)c->num_sms * c->walk_blocks_per_sm[2] * kWalkWarps;
     const bool few_groups = !c->groups_all_active || 2ull * (c->n / c->prm.ncrit) <= resident_warps;
-    const int which = ((a.eps2 == 0.0f) ? 1 : 0) + (few_groups ? 2 : 0);
+    const int which = ((a.eps2 == 0.0f) ? 1 : 0) + (few_groups ? 2 : 0) + (c->prm.order == 1 ? 4 : 0);
     const int grid = c->num_sms * c->walk_blocks_per_sm[which];
     kWalkKernels[which]<<<grid, kWalkWarps * 32, smem, c->stream>>>(a);
     c->launches += 1;

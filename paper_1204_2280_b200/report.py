@@ -6,6 +6,8 @@
               with the tree rebuilt and with the tree refreshed (bonsai_refresh_tree)
   scaling     N = 2^15 ... 2^22: time per stage (the paper's Fig. 2 quantity)
   merger      N = 2^20: the second workload (two Plummer spheres on approach) against the single sphere
+  mac         N = 2^18: theta-error-cost table of the MAC variants (geometric / tight particle-box MAC, quadrupole /
+              monopole-only), the error measured against the library's own theta = 0 walk (= direct summation)
 
 Everything runs through the C-ABI binding on cuda:0 with seeded synthetic Plummer spheres; times are CUDA-event
 stage times of the library (median of `--reps`), L2 not flushed between repetitions.  Prints one JSON document.
@@ -153,15 +155,52 @@ def merger(reps: int) -> dict:
     return {"n": n, "eps": eps, "theta": theta, "by_workload": res}
 
 
+def mac_variants(reps: int) -> dict:
+    """Row f3 (theta "sets the trade-off between speed and accuracy"): for mac_mode in {geometric, tight} and
+    order in {quadrupole, monopole}, the theta sweep of configs[1] at N = 2^18 -- interactions per particle, walk time,
+    and the force error of 4096 scattered sinks against the SAME library's theta = 0 walk of those sinks (theta = 0
+    opens everything: direct summation through the tree; the parity tests pin it to the oracle's direct sum)."""
+    cfg = W.CONFIGS["plummer_256k"]
+    n, eps = cfg["n"], cfg["eps"]
+    pm_h = W.plummer(n)
+    pm = torch.from_numpy(pm_h).cuda()
+    mask_h = W.active_mask(pm_h, 4096, "scattered")
+    mask = torch.from_numpy(mask_h).cuda()
+    sel = torch.from_numpy(np.nonzero(mask_h)[0]).cuda()
+    b0 = Bonsai(n)
+    exact = b0.step(pm, 0.0, eps, mask)[sel].double()
+    b0.sync()
+    rows = {}
+    for mac_mode, mac_name in ((0, "geometric"), (1, "tight")):
+        for order, order_name in ((2, "quadrupole"), (1, "monopole")):
+            b = Bonsai(n, mac_mode=mac_mode, order=order)
+            b.set_timing(True)
+            by_theta = {}
+            for theta in cfg["theta_sweep"]:
+                out = b.step(pm, theta, eps)
+                b.sync()
+                st = _median_stage(b, lambda: b.step(pm, theta, eps), reps)
+                pp, pc = b.interaction_totals()
+                got = out[sel].double()
+                err = (torch.linalg.norm(got[:, :3] - exact[:, :3], dim=1) / torch.linalg.norm(exact[:, :3], dim=1)).cpu().numpy()
+                by_theta[str(theta)] = {"acc_err_median": float(np.median(err)), "acc_err_p99": float(np.quantile(err, 0.99)),
+                                        "pp_per_particle": pp / n, "pc_per_particle": pc / n, "walk_ms": st["walk"],
+                                        "multipoles_ms": st["multipoles"]}
+            rows[f"{mac_name}/{order_name}"] = by_theta
+            del b
+    return {"n": n, "eps": eps, "sinks_compared": 4096, "error_reference": "theta = 0 walk of the same library",
+            "variants": rows}
+
+
 def main() -> None:
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--reps", type=int, default=5)
-    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling", "merger"), default=None)
+    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling", "merger", "mac"), default=None)
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("report: no CUDA device -- libbonsai has no CPU fallback")
     parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "scaling": scaling,
-             "merger": merger}
+             "merger": merger, "mac": mac_variants}
     doc = {k: f(args.reps) for k, f in parts.items() if args.only in (None, k)}
     print(json.dumps(doc, indent=1))
 
