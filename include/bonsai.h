@@ -66,6 +66,9 @@ typedef struct {
                             of the cell's particles, l_t = its longest side, centre = its midpoint (R28)         */
     uint32_t order;      /* [2] multipole order of a particle-cell interaction: 2 = monopole + quadrupole (R8),
                             1 = monopole only (R29); 0 = default                                                */
+    float rebuild_factor;/* [1.25] bonsai_block_tick(rebuild = -1) rebuilds the tree when the interactions per
+                            walked sink of the last walk exceed rebuild_factor x those of the first walk after the
+                            last build (R30); >= 1                                                       */
 } bonsai_params;
 
 /* Bytes of device workspace bonsai_create() needs for up to n_max particles (0 on bad arguments). */
@@ -255,13 +258,22 @@ int bonsai_kick_rungs(bonsai_ctx* ctx, float* vel_dev, const float* acc_pot_dev,
 
 /* One tick of the block scheme (R27), everything on the device, no host read-back:
  *   opening kick of the particles active at `tick`; drift of ALL particles by dt_min; force on the particles active
- *   at tick + 1 (masked walk) from a rebuilt (rebuild != 0) or refreshed (rebuild == 0, bonsai_refresh_tree) tree;
+ *   at tick + 1 (masked walk) from a rebuilt (rebuild > 0) or refreshed (rebuild == 0, bonsai_refresh_tree) tree;
  *   closing kick of those; their new rungs.
+ *   rebuild < 0: the library decides ON THE DEVICE (rebuild "only when the tree-traverse shows a considerable
+ *   decline in performance"; R30): rebuild iff the interactions per walked sink of the previous tick's walk exceed
+ *   params.rebuild_factor times those of the first tick after the last build; both kernel sequences are enqueued
+ *   behind a device flag, the one not taken returns at once.  Without a tree for this array / n it rebuilds.
  * acc_pot_dev holds every particle's force at its last force time and is updated for the walked particles only.
  * With kmax = 0 this is bonsai_leapfrog_step.  ESTATE if rebuild == 0 and no tree for this array / n exists. */
 int bonsai_block_tick(bonsai_ctx* ctx, float* pos_mass_dev, float* vel_dev, float* acc_pot_dev, uint8_t* rung_dev,
                       uint32_t n, uint64_t tick, float theta, float eps, float eta, float dt_max, uint32_t kmax,
                       int rebuild);
+
+/* R30 bookkeeping of bonsai_block_tick: decisions taken and rebuilds decided on the device since bonsai_create,
+ * the reference and the latest interactions per walked sink.  Any pointer may be NULL.  Waits for the stream. */
+int bonsai_get_rebuild_stats(bonsai_ctx* ctx, uint32_t* n_decisions, uint32_t* n_rebuilds, double* ipp_ref,
+                             double* ipp_last);
 
 /* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events around every stage from then on;
  * bonsai_get_stage_ms() waits for the stream and writes, per stage, the milliseconds SUMMED over its executions

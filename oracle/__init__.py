@@ -436,17 +436,59 @@ def kick_rungs(vel4, acc_pot, rung, mask, dt_max):
                             C.c_uint32(vel4.shape[0]), C.c_float(dt_max))
 
 
-def block_tick(pm, v4, ap, rung, tick, theta, eps, eta, dt_max, kmax, prev: Step = None, **kw):
+class RebuildPolicy:
+    """R30 (rebuild "only when the tree-traverse shows a considerable decline in performance ... an increase of
+    the average number of particle-cell and particle-particle interactions"):
+        I_t   = (sum n_pp + sum n_pc over the sinks walked in tick t) / (number of sinks walked)     (fp64)
+        I_ref = I of the first recorded walk after the last full build
+        rebuild at the start of a tick  <=>  a reference exists  and  I_last > factor I_ref          (factor fp32)
+    """
+
+    def __init__(self, factor=1.25):
+        self.factor = float(np.float32(factor))
+        self.ref = 0.0
+        self.last = 0.0
+        self.fresh = True          # no reference yet
+        self.decisions = []        # True = rebuild, one entry per decide()
+
+    def decide(self) -> bool:
+        rebuild = (not self.fresh) and self.last > self.factor * self.ref
+        self.decisions.append(bool(rebuild))
+        return rebuild
+
+    def built(self):
+        self.fresh = True
+
+    def record(self, w: WalkResult, walked_sorted: np.ndarray):
+        k = int(walked_sorted.sum())
+        if k == 0:
+            return
+        total = int(w.n_pp[walked_sorted].astype(np.int64).sum() + w.n_pc[walked_sorted].astype(np.int64).sum())
+        self.last = float(total) / float(k)
+        if self.fresh:
+            self.ref = self.last
+            self.fresh = False
+
+
+def block_tick(pm, v4, ap, rung, tick, theta, eps, eta, dt_max, kmax, prev: Step = None, policy: RebuildPolicy = None,
+               **kw):
     """One tick of the block scheme (R27), in place on pm / v4 / ap / rung.  prev: refresh this Step's tree instead
-    of rebuilding (R25).  Returns (the Step of this tick, number of active particles walked)."""
+    of rebuilding (R25).  policy: decide between the two with R30 (prev must then be the last tick's Step, or None
+    when no tree exists yet).  Returns (the Step of this tick, number of active particles walked)."""
     m0 = active_at(rung, kmax, tick)
     kick_rungs(v4, ap, rung, m0, dt_max)
     drift(pm, v4, np.float32(np.ldexp(np.float32(dt_max), -kmax)))
     m1 = active_at(rung, kmax, tick + 1)
+    if policy is not None and prev is not None and policy.decide():
+        prev = None
     if prev is None:
         s = full_step(pm, theta, eps, active_mask=m1, **kw)
+        if policy is not None:
+            policy.built()
     else:
         s = refreshed_step(prev, pm, theta, eps, active_mask=m1, **kw)
+    if policy is not None:
+        policy.record(s.walk, m1[s.perm].astype(bool))
     sel = m1[s.perm].astype(bool)
     new = np.empty((int(sel.sum()), 4), np.float64)
     new[:, :3] = s.walk.acc[sel]

@@ -31,14 +31,14 @@ SYMBOLS = (
     "bonsai_get_launch_count", "bonsai_strerror",
     "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
     "bonsai_timestep_rungs", "bonsai_active_mask", "bonsai_kick_rungs", "bonsai_block_tick",
-    "bonsai_measure_fp32_peak",
+    "bonsai_measure_fp32_peak", "bonsai_get_rebuild_stats",
 )
 
 
 class Params(C.Structure):
     _fields_ = [("nleaf", C.c_uint32), ("ncrit", C.c_uint32), ("group_mode", C.c_uint32),
                 ("cap_cells", C.c_uint32), ("group_cell", C.c_uint32), ("mac_mode", C.c_uint32),
-                ("order", C.c_uint32)]
+                ("order", C.c_uint32), ("rebuild_factor", C.c_float)]
 
 
 class CellsView(C.Structure):
@@ -101,6 +101,7 @@ def lib() -> C.CDLL:
     L.bonsai_drift.argtypes = [vp, vp, vp, u32, f32]
     L.bonsai_leapfrog_step.argtypes = [vp, vp, vp, vp, u32, f32, f32, f32]
     L.bonsai_diagnostics.argtypes = [vp, vp, vp, vp, u32, vp]
+    L.bonsai_get_rebuild_stats.argtypes = [vp, C.POINTER(u32), C.POINTER(u32), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.bonsai_measure_fp32_peak.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
     L.bonsai_strerror.argtypes = [C.c_int]
     L.bonsai_strerror.restype = C.c_char_p
@@ -131,7 +132,7 @@ def measure_fp32_peak(packed: bool = True, iters: int = 20000, stream: "torch.cu
 
 def workspace_bytes(n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
                     cap_cells: int = 0, group_cell: int = 0, mac_mode: int = 0, order: int = 2) -> int:
-    p = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order)
+    p = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order, 0.0)
     return int(lib().bonsai_workspace_bytes(n_max, C.byref(p)))
 
 
@@ -176,14 +177,15 @@ class Bonsai:
 
     def __init__(self, n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
                  cap_cells: int = 0, group_cell: int = 0, device: str | torch.device = "cuda:0",
-                 stream: "torch.cuda.Stream | None" = None, mac_mode: int = 0, order: int = 2):
+                 stream: "torch.cuda.Stream | None" = None, mac_mode: int = 0, order: int = 2,
+                 rebuild_factor: float = 0.0):
         if not torch.cuda.is_available():
             raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
         self.device = torch.device(device)
         self._L = lib()
         self.n_max = int(n_max)
         self.n = 0
-        self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order)
+        self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order, rebuild_factor)
         nbytes = int(self._L.bonsai_workspace_bytes(self.n_max, C.byref(self.params)))
         if nbytes == 0:
             raise BonsaiError(EINVAL, "bonsai_workspace_bytes")
@@ -346,15 +348,23 @@ class Bonsai:
                                              float(dt_max)), "bonsai_kick_rungs")
 
     def block_tick(self, pos_mass: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor, rung: torch.Tensor, tick: int,
-                   theta: float, eps: float, eta: float, dt_max: float, kmax: int, rebuild: bool = True) -> None:
-        """One tick of the block time-step scheme in place (bonsai_block_tick)."""
+                   theta: float, eps: float, eta: float, dt_max: float, kmax: int, rebuild: "bool | int" = True) -> None:
+        """One tick of the block time-step scheme in place (bonsai_block_tick).  rebuild: True / False, or -1 = decided
+        on the device (R30)."""
         n = pos_mass.shape[0]
         self._keep = [pos_mass]
         with torch.cuda.device(self.device):
             _check(self._L.bonsai_block_tick(self._h, self._f4(pos_mass), self._f4(vel, n), self._f4(acc_pot, n),
                                              self._u8(rung, n), n, int(tick), float(theta), float(eps), float(eta),
-                                             float(dt_max), int(kmax), int(bool(rebuild))), "bonsai_block_tick")
+                                             float(dt_max), int(kmax), -1 if (rebuild is not True and rebuild is not False and int(rebuild) < 0) else int(bool(rebuild))), "bonsai_block_tick")
         self.n = n
+
+    def rebuild_stats(self) -> dict:
+        nd, nr, ref, last = C.c_uint32(0), C.c_uint32(0), C.c_double(0), C.c_double(0)
+        _check(self._L.bonsai_get_rebuild_stats(self._h, C.byref(nd), C.byref(nr), C.byref(ref), C.byref(last)),
+               "bonsai_get_rebuild_stats")
+        return {"n_decisions": int(nd.value), "n_rebuilds": int(nr.value), "ipp_ref": float(ref.value),
+                "ipp_last": float(last.value)}
 
     def sync(self) -> None:
         _check(self._L.bonsai_sync(self._h), "bonsai_sync")

@@ -39,13 +39,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
         newest = max(os.path.getmtime(p) for p in _deps())
         if os.path.getmtime(LIB) >= newest:
             return LIB
-    cmd = [_nvcc(), *ARCH, "-O3", "-std=c++17", "-lineinfo",
-           "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "-cudart", "static",
-           "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+    # one nvcc per translation unit, in parallel (objects under build/, git-ignored), then one link
+    from concurrent.futures import ThreadPoolExecutor
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    flags = [*ARCH, "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-O2,-Wall",
+             "-I", os.path.join(ROOT, "include"), "-I", CSRC]
     if verbose:
-        cmd += ["-Xptxas", "-v"]
-    cmd += sources() + ["-o", LIB]
-    subprocess.run(cmd, check=True)
+        flags += ["-Xptxas", "-v"]
+    nvcc = _nvcc()
+
+    def compile_one(src: str) -> str:
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        subprocess.run([nvcc, *flags, "-c", src, "-o", obj], check=True)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        objs = list(ex.map(compile_one, sources()))
+    subprocess.run([nvcc, *ARCH, "-shared", "-cudart", "static", *objs, "-o", LIB], check=True)
     return LIB
 
 

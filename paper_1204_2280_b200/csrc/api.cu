@@ -30,8 +30,9 @@ struct Carver {
 
 bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out) {
     bonsai_params p;
-    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0; p.mac_mode = 0; p.order = 2;
+    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0; p.mac_mode = 0; p.order = 2; p.rebuild_factor = 0.0f;
     if (in) {
+        p.rebuild_factor = in->rebuild_factor;
         p.mac_mode = in->mac_mode;
         if (in->order) p.order = in->order;
         if (in->nleaf) p.nleaf = in->nleaf;
@@ -52,6 +53,8 @@ bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out)
     if (p.ncrit < 1 || p.ncrit > (uint32_t)kMaxNcrit) return false;
     if (p.group_mode > 2) return false;
     if (p.mac_mode > 1 || p.order < 1 || p.order > 2) return false;
+    if (p.rebuild_factor == 0.0f) p.rebuild_factor = 1.25f;
+    if (!(p.rebuild_factor >= 1.0f) || std::isinf(p.rebuild_factor)) return false;
     if (p.cap_cells < 1 || p.cap_cells >= (1u << 29)) return false;  // walk stack entries pack the id into 29 bits
     *out = p;
     return true;
@@ -191,6 +194,8 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
         return BONSAI_ECUDA;
     }
     c.device = dev;
+    c.gate = Gate{nullptr, 0u};
+    c.tree_auto = false;
     // kernel attributes and occupancy are per device: set for every context (idempotent), never behind a
     // process-wide flag
     if (walk_prepare(&c) != cudaSuccess || sort_prepare(&c) != cudaSuccess) {
@@ -220,13 +225,8 @@ int bonsai_load(bonsai_ctx* h, const float* pos_mass_dev, uint32_t n) {
     return BONSAI_OK;
 }
 
-int bonsai_build_tree(bonsai_ctx* h) {
-    if (!h) return BONSAI_EINVAL;
-    Ctx* c = &h->c;
-    if (c->state < 1) return BONSAI_ESTATE;
-    // the sticky status reports the work since the last build: a capacity overflow of an earlier step (reported by
-    // the bonsai_sync of that step) must not poison this one
-    BONSAI_TRY(stage_recover(c));
+// Stages a0..a4 (everything of bonsai_build_tree but the groups); every launch honours c->gate.
+static int build_chain(Ctx* c) {
     { StageTimer t(c, 0); BONSAI_TRY(stage_bbox(c)); }
     { StageTimer t(c, 1); BONSAI_TRY(stage_keys(c)); }
     { StageTimer t(c, 2); BONSAI_TRY(stage_sort(c)); }
@@ -236,9 +236,43 @@ int bonsai_build_tree(bonsai_ctx* h) {
         BONSAI_TRY(stage_sort_ties(c));
     }
     { StageTimer t(c, 4); BONSAI_TRY(stage_build(c)); }
+    return BONSAI_OK;
+}
+
+int bonsai_build_tree(bonsai_ctx* h) {
+    if (!h) return BONSAI_EINVAL;
+    Ctx* c = &h->c;
+    if (c->state < 1) return BONSAI_ESTATE;
+    // the sticky status reports the work since the last build: a capacity overflow of an earlier step (reported by
+    // the bonsai_sync of that step) must not poison this one
+    BONSAI_TRY(stage_recover(c));
+    int rc;
+    if ((rc = build_chain(c)) != BONSAI_OK) return rc;
     { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
     c->tree_n = c->n;
     c->tree_refreshed = false;
+    c->tree_auto = false;
+    c->state = 2;
+    return BONSAI_OK;
+}
+
+// R30: rebuild or refresh, decided on the device from the interaction totals of the last recorded walk.  Both
+// sequences are enqueued behind opposite gates on Control::rebuild_flag; there is no host read-back.
+static int build_or_refresh_on_device(Ctx* c) {
+    BONSAI_TRY(stage_rebuild_decide(c, c->prm.rebuild_factor));
+    Buffers& b = c->b;
+    c->gate = Gate{&b.ctl->rebuild_flag, 1u};
+    int rc = build_chain(c);
+    c->gate = Gate{&b.ctl->rebuild_flag, 0u};
+    if (rc == BONSAI_OK) {
+        StageTimer t(c, 3);
+        if (stage_reorder(c, false) != cudaSuccess) rc = BONSAI_ECUDA;
+    }
+    c->gate = Gate{nullptr, 0u};
+    if (rc != BONSAI_OK) return rc;
+    { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
+    c->tree_refreshed = false;
+    c->tree_auto = true;  // the multipole pass asks the device flag whether the cell sides grow (R25)
     c->state = 2;
     return BONSAI_OK;
 }
@@ -250,6 +284,7 @@ int bonsai_refresh_tree(bonsai_ctx* h) {
     { StageTimer t(c, 3); BONSAI_TRY(stage_reorder(c, false)); }
     { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
     c->tree_refreshed = true;
+    c->tree_auto = false;
     c->state = 2;
     return BONSAI_OK;
 }
@@ -407,7 +442,9 @@ int bonsai_block_tick(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, float*
         std::isinf(eps) || std::isinf(dt_max))
         return BONSAI_EINVAL;
     Ctx* c = &h->c;
-    if (!rebuild && (c->tree_n != n || c->pos_mass != reinterpret_cast<const float4*>(pos_mass_dev))) return BONSAI_ESTATE;
+    const bool have_tree = c->tree_n == n && c->pos_mass == reinterpret_cast<const float4*>(pos_mass_dev);
+    if (rebuild == 0 && !have_tree) return BONSAI_ESTATE;
+    if (rebuild < 0 && !have_tree) rebuild = 1;  // R30 needs a tree to decide about
     float4* vel = reinterpret_cast<float4*>(vel_dev);
     const float4* acc = reinterpret_cast<const float4*>(acc_pot_dev);
     uint8_t* mask = c->b.tick_mask;
@@ -421,9 +458,12 @@ int bonsai_block_tick(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, float*
     }
     BONSAI_TRY(stage_active_mask(c, rung_dev, n, kmax, tick + 1, mask));
     if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
-    if ((rc = rebuild ? bonsai_build_tree(h) : bonsai_refresh_tree(h)) != BONSAI_OK) return rc;
+    if (rebuild < 0) rc = build_or_refresh_on_device(c);
+    else rc = rebuild ? bonsai_build_tree(h) : bonsai_refresh_tree(h);
+    if (rc != BONSAI_OK) return rc;
     if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
     if ((rc = bonsai_walk(h, theta, eps, mask, acc_pot_dev)) != BONSAI_OK) return rc;
+    BONSAI_TRY(stage_walk_stats(c));  // R30: interactions per walked sink; the first walk after a build is the reference
     {
         StageTimer t(c, 8);
         BONSAI_TRY(stage_kick_rungs(c, vel, acc, rung_dev, mask, n, dt_max));
@@ -534,6 +574,19 @@ int bonsai_get_interaction_totals(bonsai_ctx* h, uint64_t* sum_pp, uint64_t* sum
     if (cudaStreamSynchronize(h->c.stream) != cudaSuccess) return BONSAI_ECUDA;
     *sum_pp = v[0];
     *sum_pc = v[1];
+    return BONSAI_OK;
+}
+
+int bonsai_get_rebuild_stats(bonsai_ctx* h, uint32_t* n_decisions, uint32_t* n_rebuilds, double* ipp_ref, double* ipp_last) {
+    if (!h) return BONSAI_EINVAL;
+    Control host;
+    if (cudaMemcpyAsync(&host, h->c.b.ctl, sizeof(Control), cudaMemcpyDeviceToHost, h->c.stream) != cudaSuccess)
+        return BONSAI_ECUDA;
+    if (cudaStreamSynchronize(h->c.stream) != cudaSuccess) return BONSAI_ECUDA;
+    if (n_decisions) *n_decisions = host.n_decisions;
+    if (n_rebuilds) *n_rebuilds = host.n_rebuilds;
+    if (ipp_ref) *ipp_ref = host.ipp_ref;
+    if (ipp_last) *ipp_last = host.ipp_last;
     return BONSAI_OK;
 }
 

@@ -61,11 +61,25 @@ struct Control {
     uint32_t diag_ticket;      // last-block-done counter of k_diagnostics
     uint32_t sort_fallback;    // set by k_sort_ties when a run of equal (hi, mid) is too long: the guarded chain runs
     uint32_t recover_ticket;   // last-block-done counter of k_recover
-    uint32_t pad1[2];
+    uint32_t rebuild_flag;     // R30: decision of k_rebuild_decide for the current tick (1 = rebuild, 0 = refresh)
+    uint32_t tree_fresh;       // R30: set by a build; the next recorded walk becomes the reference and clears it
     uint32_t level_offsets[32];  // first cell of level L; [31] = n_cells
     unsigned long long sum_pp;   // interaction totals of the last walk (sink-source pairs)
     unsigned long long sum_pc;
+    double ipp_ref;              // R30: interactions per walked sink of the first recorded walk after the last build
+    double ipp_last;             // R30: ... of the last recorded walk
+    uint32_t n_rebuilds;         // R30: rebuilds decided on the device since bonsai_create
+    uint32_t n_decisions;
 };
+
+// A launch that only does its work when a device flag has a given value.  The flag is written by an earlier kernel
+// on the same stream (k_sort_ties: the sort's fallback chain; k_rebuild_decide: R30), so a data-dependent choice
+// between two kernel sequences needs no host read-back: both are enqueued, one of them returns at once.
+struct Gate {
+    const uint32_t* flag;      // nullptr: always open
+    uint32_t want;
+};
+__device__ __forceinline__ bool gate_closed(const Gate g) { return g.flag != nullptr && __ldcg(g.flag) != g.want; }
 
 // Walk layout of a cell, two 32-byte records (one DRAM/L2 sector each):
 //   CellMac : what the opening test and the monopole need + the links
@@ -147,6 +161,8 @@ struct Ctx {
     uint64_t launches;
     int num_sms;
     int device;                // the CUDA device the context was created on
+    Gate gate;                 // applied to every launch of the build chain (bbox .. tree) while it is set (R30)
+    bool tree_auto;            // the tree on the device was rebuilt OR refreshed by a device-side decision (R30)
     int walk_blocks_per_sm[8]; // occupancy of the k_walk instances on this device (set in bonsai_create)
 };
 
@@ -165,6 +181,8 @@ cudaError_t cells_qraw(Ctx* c);  // fills c_qraw from c_mom (introspection)
 cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out);
 cudaError_t walk_prepare(Ctx* c);  // per-device kernel attributes and occupancy (bonsai_create)
 cudaError_t sort_prepare(Ctx* c);
+cudaError_t stage_rebuild_decide(Ctx* c, float factor);  // R30 (policy.cu)
+cudaError_t stage_walk_stats(Ctx* c);
 cudaError_t stage_recover(Ctx* c); // guarded: re-zeroes the arrival counters after a capacity overflow, clears the status
 size_t walk_smem_bytes(uint32_t nleaf);
 cudaError_t stage_kick(Ctx* c, float4* vel, const float4* acc, uint32_t n, float h, const uint8_t* mask);

@@ -39,7 +39,7 @@ __device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], c
                                            const Control* __restrict__ ctl, uint32_t link_first, uint32_t link_info,
                                            double* __restrict__ c_mom, float* __restrict__ c_box,
                                            CellMac* __restrict__ c_mac, CellQuad* __restrict__ c_quad,
-                                           float* __restrict__ c_qraw) {
+                                           float* __restrict__ c_qraw, const bool grow) {
     // geometric centre: integer cell coordinate = top L bits of the quantised coordinate of any member (R8)
     double l = ldexp(ctl->side, -L);
     double g[3];
@@ -65,7 +65,7 @@ __device__ __forceinline__ void store_cell(const Mom& q, const float (&mn)[3], c
                 l = fmax(l, __dadd_rn((double)mx[d], -(double)mn[d]));
                 g[d] = __dmul_rn(0.5, __dadd_rn((double)mn[d], (double)mx[d]));
             }
-        } else {
+        } else if (grow) {
             double e = 0.0;
 #pragma unroll
             for (int d = 0; d < 3; ++d) e = fmax(e, fmax(__dadd_rn(g[d], -(double)mn[d]), __dadd_rn((double)mx[d], -g[d])));
@@ -114,7 +114,10 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
                                                     const uint32_t* __restrict__ klo, double* __restrict__ c_mom,
                                                     CellMac* __restrict__ c_mac, CellQuad* __restrict__ c_quad,
                                                     float* __restrict__ c_qraw, float* __restrict__ c_box,
-                                                    uint32_t* __restrict__ c_arrived) {
+                                                    uint32_t* __restrict__ c_arrived, const Gate grow_gate) {
+    // R25 growth of the cell side applies to a REFRESHED tree only; whether this tree was refreshed may have been
+    // decided on the device (R30): the gate is open (or absent) when it was
+    const bool grow = !gate_closed(grow_gate);
     uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= min(ctl->n_cells, cap_cells)) return;
     if (t.n_child[c] != 0) return;  // internal cells are produced by their last child
@@ -155,7 +158,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
             }
         }
         store_cell<kBox, kTight>(q, mn, mx, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f,
-                   kLeafBit | cnt, c_mom, c_box, c_mac, c_quad, c_qraw);
+                   kLeafBit | cnt, c_mom, c_box, c_mac, c_quad, c_qraw, grow);
     }
     for (;;) {
         const uint32_t p = t.parent[c];
@@ -216,7 +219,7 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
         }
         const uint32_t f = t.first[p];
         store_cell<kBox, kTight>(q, mn, mx, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc,
-                   c_mom, c_box, c_mac, c_quad, c_qraw);
+                   c_mom, c_box, c_mac, c_quad, c_qraw, grow);
         c = p;
     }
 }
@@ -264,12 +267,14 @@ cudaError_t stage_multipoles(Ctx* c) {
     TreeView t{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
     const dim3 grid(div_up(c->cap_cells, 128));
     using Kernel = void (*)(const Control*, uint32_t, TreeView, const float4*, const uint32_t*, const uint32_t*, const uint32_t*,
-                            double*, CellMac*, CellQuad*, float*, float*, uint32_t*);
-    const Kernel k = (c->prm.mac_mode == 1) ? (Kernel)k_multipoles<true, true>
-                     : c->tree_refreshed    ? (Kernel)k_multipoles<true, false>
-                                            : (Kernel)k_multipoles<false, false>;
+                            double*, CellMac*, CellQuad*, float*, float*, uint32_t*, Gate);
+    const Kernel k = (c->prm.mac_mode == 1)              ? (Kernel)k_multipoles<true, true>
+                     : (c->tree_refreshed || c->tree_auto) ? (Kernel)k_multipoles<true, false>
+                                                           : (Kernel)k_multipoles<false, false>;
+    // a tree handled by the device-side rebuild decision (R30) was refreshed iff rebuild_flag == 0
+    const Gate grow = c->tree_auto ? Gate{&b.ctl->rebuild_flag, 0u} : Gate{nullptr, 0u};
     k<<<grid, 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1], b.key[s][2], b.c_mom,
-                                   b.c_mac, b.c_quad, b.c_qraw, b.c_box, b.c_arrived);
+                                   b.c_mac, b.c_quad, b.c_qraw, b.c_box, b.c_arrived, grow);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -22,9 +22,10 @@ __device__ __forceinline__ void warp_minmax(float (&mn)[3], float (&mx)[3]) {
 }
 
 __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, uint32_t n, float* __restrict__ partial,
-                                              Control* __restrict__ ctl) {
+                                              Control* __restrict__ ctl, const Gate gate) {
     __shared__ float s_mn[8][3], s_mx[8][3];
     __shared__ bool s_last;
+    if (gate_closed(gate)) return;
     float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         float4 p = __ldg(&pos[i]);
@@ -119,8 +120,9 @@ __device__ __forceinline__ void morton_words(const float4 p, const float lox, co
 __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict__ pos, uint32_t n,
                                                        const Control* __restrict__ ctl, uint32_t* __restrict__ khi,
                                                        uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
-                                                       uint32_t* __restrict__ ghist) {
+                                                       uint32_t* __restrict__ ghist, const Gate gate) {
     __shared__ uint32_t h[kSortPasses * kRadix];
+    if (gate_closed(gate)) return;
     for (int k = threadIdx.x; k < kSortPasses * kRadix; k += kKeysThreads) h[k] = 0;
     __syncthreads();
     const float scale = ctl->scale, lox = ctl->lo[0], loy = ctl->lo[1], loz = ctl->lo[2];
@@ -155,9 +157,14 @@ __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict_
 }
 
 // exclusive scan of each pass's histogram: ghist[p][d] <- sum_{d' < d} ghist[p][d'].  One block per pass.
-__global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ ghist, Control* __restrict__ ctl) {
+__global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ ghist, Control* __restrict__ ctl,
+                                                       const Gate gate) {
     __shared__ uint32_t wsum[kRadix / 32];
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->sort_fallback = 0;
+    if (gate_closed(gate)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        ctl->sort_fallback = 0;
+        ctl->tree_fresh = 1;  // R30: a new tree is being built; the next recorded walk is its reference
+    }
     uint32_t* h = ghist + blockIdx.x * kRadix;
     uint32_t v = h[threadIdx.x];
     uint32_t x = v;
@@ -216,6 +223,7 @@ struct SortPass {
     unsigned long long* look;  // [n_tiles][kRadix]
     uint32_t* ticket;
     const uint32_t* guard;     // nullptr, or a device flag: the pass only runs when it is non-zero (fallback chain)
+    Gate gate;                 // and only when this gate is open (R30)
     uint32_t n, n_tiles, epoch;
     int shift;
 };
@@ -248,7 +256,8 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
     __shared__ uint32_t s_tile;
     __shared__ uint32_t s_wsum[kWarps];
     const int tid = threadIdx.x, l = tid & 31, w = tid >> 5;
-    if (a.guard != nullptr && __ldg(a.guard) == 0u) return;  // uniform over the grid: the flag was set before the launch
+    if (gate_closed(a.gate)) return;
+    if (a.guard != nullptr && __ldcg(a.guard) == 0u) return;  // uniform over the grid: the flag was set before the launch
 
     if (tid == 0) {
         const uint32_t t = atomicAdd(a.ticket, 1u);
@@ -450,8 +459,9 @@ __global__ void __launch_bounds__(256) k_reorder(const float4* __restrict__ pos,
                                                  uint32_t n, const Control* __restrict__ ctl,
                                                  float4* __restrict__ sorted_pos, uint32_t* __restrict__ khi,
                                                  uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
-                                                 const uint32_t* __restrict__ guard) {
-    if (guard != nullptr && __ldg(guard) == 0u) return;
+                                                 const uint32_t* __restrict__ guard, const Gate gate) {
+    if (gate_closed(gate)) return;
+    if (guard != nullptr && __ldcg(guard) == 0u) return;
     const float lox = ctl->lo[0], loy = ctl->lo[1], loz = ctl->lo[2], scale = ctl->scale;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const float4 p = __ldg(&pos[__ldg(&perm[i])]);
@@ -468,7 +478,7 @@ __global__ void __launch_bounds__(256) k_reorder(const float4* __restrict__ pos,
 // ------------------------------------------------------------------------------------------------
 cudaError_t stage_bbox(Ctx* c) {
     uint32_t blocks = min(min(div_up(c->n, 256 * 8), (uint32_t)(c->num_sms * 8)), (uint32_t)kBboxMaxBlocks);
-    k_bbox<<<blocks, 256, 0, c->stream>>>(c->pos_mass, c->n, c->b.bbox_partial, c->b.ctl);
+    k_bbox<<<blocks, 256, 0, c->stream>>>(c->pos_mass, c->n, c->b.bbox_partial, c->b.ctl, c->gate);
     c->launches += 1;
     return cudaGetLastError();
 }
@@ -479,7 +489,7 @@ cudaError_t stage_keys(Ctx* c) {
     if (e != cudaSuccess) return e;
     const uint32_t blocks = min(div_up(c->n, kKeysThreads), (uint32_t)(c->num_sms * 2));
     k_keys<<<blocks, kKeysThreads, 0, c->stream>>>(c->pos_mass, c->n, b.ctl, b.key[0][0], b.key[0][1], b.key[0][2],
-                                                   b.ghist);
+                                                   b.ghist, c->gate);
     c->launches += 1;
     return cudaGetLastError();
 }
@@ -521,7 +531,9 @@ __device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, co
 // side); a particle that ties with its successor but not with its predecessor heads a run.
 __global__ void __launch_bounds__(256) k_sort_ties(const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
                                                    uint32_t* __restrict__ klo, uint32_t* __restrict__ perm,
-                                                   float4* __restrict__ sorted_pos, uint32_t n, Control* __restrict__ ctl) {
+                                                   float4* __restrict__ sorted_pos, uint32_t n, Control* __restrict__ ctl,
+                                                   const Gate gate) {
+    if (gate_closed(gate)) return;
     const uint32_t i0 = 4u * (blockIdx.x * blockDim.x + threadIdx.x);
     if (i0 >= n) return;
     uint32_t h[6], m[6];  // positions i0 - 1 .. i0 + 4; out-of-range slots get a value no key has
@@ -573,6 +585,7 @@ static cudaError_t sort_chain(Ctx* c, int first_pass, int first_out, const uint3
     a.look = b.look;
     a.ticket = &b.ctl->sort_ticket;
     a.guard = guard;
+    a.gate = c->gate;
     int cur = first_out ^ 1;
     for (int p = first_pass; p < kSortPasses; ++p) {
         if (c->sort_epoch >= (1u << 30) - 1) {  // 30-bit epoch about to wrap: forget every stale entry
@@ -601,7 +614,7 @@ static cudaError_t sort_chain(Ctx* c, int first_pass, int first_out, const uint3
 // The sort proper: six passes over the mid and hi words (the lo word almost never decides the order, see k_sort_ties).
 cudaError_t stage_sort(Ctx* c) {
     Buffers& b = c->b;
-    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist, b.ctl);
+    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist, b.ctl, c->gate);
     c->launches += 1;
     c->perm = b.idx[0];
     return sort_chain(c, 3, 1, nullptr);  // outputs 1, 0, 1, 0, 1, 0
@@ -612,7 +625,7 @@ static void launch_reorder(Ctx* c, bool write_keys, const uint32_t* guard) {
     // the guarded instance normally returns at once: keep its grid small
     const uint32_t blocks = guard ? (uint32_t)c->num_sms * 8u : div_up(c->n, 256);
     k_reorder<<<blocks, 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos,
-                                             write_keys ? b.key[1][0] : nullptr, b.key[1][1], b.key[1][2], guard);
+                                             write_keys ? b.key[1][0] : nullptr, b.key[1][1], b.key[1][2], guard, c->gate);
     c->launches += 1;
 }
 
@@ -628,7 +641,7 @@ cudaError_t stage_reorder(Ctx* c, bool write_keys) {
 cudaError_t stage_sort_ties(Ctx* c) {
     Buffers& b = c->b;
     k_sort_ties<<<div_up(div_up(c->n, 4), 256), 256, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
-                                                          b.ctl);
+                                                          b.ctl, c->gate);
     c->launches += 1;
     const uint32_t* guard = &b.ctl->sort_fallback;
     cudaError_t e = sort_chain(c, 0, 0, guard);  // outputs 0, 1, 0, 1, 0, 1, 0, 1, 0

@@ -36,7 +36,8 @@ __device__ __forceinline__ int common_digits(uint32_t ahi, uint32_t amid, uint32
 
 __global__ void __launch_bounds__(256) k_tree_lcp(const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
                                                   const uint32_t* __restrict__ klo, uint32_t n,
-                                                  int8_t* __restrict__ lcp) {
+                                                  int8_t* __restrict__ lcp, const Gate gate) {
+    if (gate_closed(gate)) return;
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i > n) return;
     int v = -1;
@@ -61,8 +62,9 @@ __device__ __forceinline__ uint32_t tree_item(uint32_t block, int w, int r, int 
 
 __global__ void __launch_bounds__(kTreeThreads) k_tree_levels(const int8_t* __restrict__ lcp, uint32_t n, int nleaf,
                                                               uint32_t n_blocks, int8_t* __restrict__ leaf_level,
-                                                              uint32_t* __restrict__ blk_level_count) {
+                                                              uint32_t* __restrict__ blk_level_count, const Gate gate) {
     constexpr int H = kMaxNleaf;
+    if (gate_closed(gate)) return;
     __shared__ int8_t s_lcp[kTreeTile + 2 * H + 1];
     __shared__ uint32_t s_cnt[kLevelSlots];
     const long long base = (long long)blockIdx.x * kTreeTile;
@@ -105,8 +107,9 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_levels(const int8_t* __re
 // into level offsets and n_cells.
 __global__ void __launch_bounds__(256) k_tree_scan_levels(uint32_t* __restrict__ blk_level_count, uint32_t n_blocks,
                                                           uint32_t* __restrict__ level_total, Control* __restrict__ ctl,
-                                                          uint32_t cap_cells) {
+                                                          uint32_t cap_cells, const Gate gate) {
     __shared__ uint32_t wsum[8];
+    if (gate_closed(gate)) return;
     __shared__ uint32_t carry;
     __shared__ bool s_last;
     uint32_t* row = blk_level_count + (size_t)blockIdx.x * n_blocks;
@@ -163,8 +166,9 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_emit(const int8_t* __rest
                                                             uint32_t n_blocks,
                                                             const uint32_t* __restrict__ blk_level_prefix,
                                                             const Control* __restrict__ ctl, uint32_t cap_cells,
-                                                            CellArrays ca) {
+                                                            CellArrays ca, const Gate gate) {
     constexpr int kWarps = kTreeThreads / 32;
+    if (gate_closed(gate)) return;
     __shared__ uint32_t s_pre[kWarps][kTreeItems][kLevelSlots];
     for (int k = threadIdx.x; k < kWarps * kTreeItems * kLevelSlots; k += kTreeThreads) (&s_pre[0][0][0])[k] = 0;
     __syncthreads();
@@ -245,7 +249,8 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_emit(const int8_t* __rest
 }
 
 __global__ void __launch_bounds__(256) k_tree_finalize(const Control* __restrict__ ctl, uint32_t cap_cells,
-                                                       CellArrays ca) {
+                                                       CellArrays ca, const Gate gate) {
+    if (gate_closed(gate)) return;
     // grid-stride: the number of cells is only known on the device, a grid sized for cap_cells would be mostly empty
     const uint32_t n_cells = min(ctl->n_cells, cap_cells);
     for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += gridDim.x * blockDim.x) {
@@ -261,14 +266,14 @@ cudaError_t stage_build(Ctx* c) {
     const int s = c->sorted_buf;
     const uint32_t n_blocks = div_up(n + 1, kTreeTile);
     CellArrays ca{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
-    k_tree_lcp<<<div_up(n + 1, 256), 256, 0, c->stream>>>(b.key[s][0], b.key[s][1], b.key[s][2], n, b.lcp);
+    k_tree_lcp<<<div_up(n + 1, 256), 256, 0, c->stream>>>(b.key[s][0], b.key[s][1], b.key[s][2], n, b.lcp, c->gate);
     k_tree_levels<<<n_blocks, kTreeThreads, 0, c->stream>>>(b.lcp, n, (int)c->prm.nleaf, n_blocks, b.leaf_level,
-                                                            b.blk_level_count);
+                                                            b.blk_level_count, c->gate);
     k_tree_scan_levels<<<kMaxLevel + 1, 256, 0, c->stream>>>(b.blk_level_count, n_blocks, b.level_total, b.ctl,
-                                                             c->cap_cells);
+                                                             c->cap_cells, c->gate);
     k_tree_emit<<<n_blocks, kTreeThreads, 0, c->stream>>>(b.lcp, b.leaf_level, n, n_blocks, b.blk_level_count, b.ctl,
-                                                          c->cap_cells, ca);
-    k_tree_finalize<<<min(div_up(c->cap_cells, 256), (uint32_t)c->num_sms * 16u), 256, 0, c->stream>>>(b.ctl, c->cap_cells, ca);
+                                                          c->cap_cells, ca, c->gate);
+    k_tree_finalize<<<min(div_up(c->cap_cells, 256), (uint32_t)c->num_sms * 16u), 256, 0, c->stream>>>(b.ctl, c->cap_cells, ca, c->gate);
     c->launches += 5;
     return cudaGetLastError();
 }

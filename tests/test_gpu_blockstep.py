@@ -112,6 +112,43 @@ def test_block_ticks_follow_the_oracle(rebuild_every):
            dv_median_over_vrms=float(np.median(dv) / vrms), dv_max_over_vrms=float(dv.max() / vrms))
 
 
+def test_device_side_rebuild_decision_follows_the_oracle_policy():
+    """R30: bonsai_block_tick(rebuild = -1) decides on the device, from the interaction totals of the last
+    walk, whether the tick rebuilds or refreshes the tree -- no host read-back.  Tick by tick the number of rebuilds
+    and the recorded interactions per walked sink must equal those of oracle.block_tick(policy=RebuildPolicy), and the
+    run must contain both kinds of tick."""
+    n, theta, eps, eta, dt_max, kmax, factor = 8192, 0.75, 0.01, 0.3, 1 / 4, 2, 1.02
+    pm, vel = W.plummer(n, with_velocities=True)
+    b = Bonsai(n, rebuild_factor=factor)
+    p_d, v_d = _dev(pm), _dev(O._vel4(vel))
+    a_d = b.step(p_d, theta, eps).clone()
+    r_d = b.timestep_rungs(a_d, eta, eps, dt_max, kmax)
+    p, v = pm.copy(), O._vel4(vel)
+    ap = O.force_f32(p, theta, eps)
+    r = O.rungs(ap, eta, eps, dt_max, kmax)
+    assert (r_d.cpu().numpy() != r).mean() < 1e-3
+    # the context already holds a tree for p_d (built by b.step): the first tick decides; without a reference it refreshes
+    pol = O.RebuildPolicy(factor)
+    prev = O.build(pm)
+    for tick in range(12):
+        b.block_tick(p_d, v_d, a_d, r_d, tick, theta, eps, eta, dt_max, kmax, rebuild=-1)
+        s, na = O.block_tick(p, v, ap, r, tick, theta, eps, eta, dt_max, kmax, prev=prev, policy=pol)
+        prev = s
+        st = b.rebuild_stats()
+        assert st["n_decisions"] == len(pol.decisions) and st["n_rebuilds"] == sum(pol.decisions), (tick, st, pol.decisions)
+        assert np.isclose(st["ipp_last"], pol.last, rtol=2e-3) and np.isclose(st["ipp_ref"], pol.ref, rtol=2e-3)
+        # the tree on the device is the oracle's: rebuilt (new permutation) or frozen (old one)
+        assert np.array_equal(b.perm(), s.perm), tick
+    assert any(pol.decisions) and not all(pol.decisions), pol.decisions
+    b.sync()
+    assert (r_d.cpu().numpy() != r).mean() < 1e-2
+    dx = np.abs(p_d.cpu().numpy()[:, :3].astype(np.float64) - p[:, :3]).max(axis=1)
+    assert np.median(dx) <= 2e-7 and np.quantile(dx, 0.97) <= 1e-5
+    from test_gpu_parity import record
+    record("device-side rebuild decision", ticks=12, rebuilds=int(sum(pol.decisions)), decisions=[int(d) for d in pol.decisions],
+           ipp_ref=float(pol.ref), ipp_last=float(pol.last))
+
+
 def test_block_tick_errors():
     n = 1000
     pm, vel = W.plummer(n, with_velocities=True)

@@ -100,3 +100,58 @@ def test_refreshed_force_stays_accurate_and_costs_more(base):
         # and it costs more, increasingly so
         assert cost["refresh", t] > cost["fresh", t]
     assert cost["refresh", 0.1] / cost["fresh", 0.1] > cost["refresh", 0.02] / cost["fresh", 0.02]
+
+
+def test_rebuild_policy_fires_after_the_drift_and_not_before(base):
+    """R30: the rule compares the interactions per walked sink of the last walk with those of the first walk
+    after the last build.  Pinned on the very drift that test_refreshed_force_stays_accurate_and_costs_more shows to
+    raise the cost: fed with a fresh walk (reference) and then refreshed walks after growing drifts, the policy stays
+    quiet while the ratio is below the factor and fires once it is above -- the ratios recomputed here from the
+    walk counts by numpy."""
+    pm, vel, s = base
+    pol = O.RebuildPolicy(factor=1.25)
+    assert pol.decide() is False                       # no reference yet: never rebuild
+    everyone = np.ones(N, bool)
+    pol.record(s.walk, everyone)
+    ref = (s.walk.n_pp.astype(np.float64).sum() + s.walk.n_pc.astype(np.float64).sum()) / N
+    assert pol.ref == ref and pol.last == ref and pol.fresh is False
+    assert pol.decide() is False                       # ratio 1
+    fired = []
+    for t in (0.01, 0.05, 0.2, 0.5):
+        r = O.refreshed_step(s, _drifted(pm, vel, t), THETA, EPS)
+        pol.record(r.walk, everyone)
+        ratio = (r.walk.n_pp.astype(np.float64).sum() + r.walk.n_pc.astype(np.float64).sum()) / N / ref
+        assert pol.ref == ref                          # the reference is the walk after the build, not a later one
+        fired.append((ratio, pol.decide()))
+        assert fired[-1][1] == (ratio > float(np.float32(1.25)))
+    assert fired[0][1] is False and fired[-1][1] is True, fired
+    assert all(fired[k][0] < fired[k + 1][0] for k in range(3)), fired     # the cost grows with the drift
+    # a rebuild resets the reference
+    pol.built()
+    f = O.full_step(_drifted(pm, vel, 0.5), THETA, EPS)
+    pol.record(f.walk, everyone)
+    assert pol.decide() is False and pol.ref < fired[-1][0] * ref
+
+
+def test_block_ticks_with_the_policy_rebuild_when_it_says_so():
+    """oracle.block_tick(policy=...) rebuilds exactly at the ticks the policy fires, refreshes otherwise, and a
+    masked tick records only the walked sinks."""
+    n, theta, eps, eta, dt_max, kmax = 2048, 0.75, 0.01, 0.3, 1 / 4, 2
+    pm, vel = W.plummer(n, with_velocities=True)
+    p, v = pm.copy(), O._vel4(vel)
+    ap = O.force_f32(p, theta, eps)
+    r = O.rungs(ap, eta, eps, dt_max, kmax)
+    pol = O.RebuildPolicy(factor=1.02)
+    prev = None
+    kinds = []
+    for tick in range(12):
+        s, na = O.block_tick(p, v, ap, r, tick, theta, eps, eta, dt_max, kmax, prev=prev, policy=pol)
+        fresh_tree = np.array_equal(s.lo, O.box(p)[0]) and np.array_equal(s.perm, O.sort(O.keys(p, *O.box(p))))
+        kinds.append(fresh_tree)
+        prev = s
+    assert kinds[0] is True                               # no tree yet: built
+    assert len(pol.decisions) == 11                       # one decision per tick that had a tree
+    for k, d in enumerate(pol.decisions):                 # a fired decision means a fresh sort of the CURRENT positions
+        if d:
+            assert kinds[k + 1]
+    assert any(pol.decisions) and not all(pol.decisions)
