@@ -121,8 +121,9 @@ int bonsai_walk(bonsai_ctx* ctx, float theta, float eps, const uint8_t* active_m
 /* One full force step for a caller whose particles live in HOST memory (the end-to-end path of bench.py):
  * copies pos_mass_host (float4[n]; pinned memory recommended) to a staging buffer in the workspace, runs
  * bonsai_load .. bonsai_walk exactly as above, copies acc_pot (float4[n], load order) back and WAITS for the
- * stream.  active_mask_host: host u8[n] or NULL; with a mask, acc_pot_host_out is also read (entries of inactive
- * particles are returned unchanged).  Returns what bonsai_sync() returns, or EINVAL / ECUDA. */
+ * stream.  active_mask_host: host u8[n] or NULL; with a mask, entries of inactive particles are returned unchanged.
+ * Both directions are staged through the workspace (one copy each way, 16 n bytes each).
+ * Returns what bonsai_sync() returns, or EINVAL / ECUDA. */
 int bonsai_step_host(bonsai_ctx* ctx, const float* pos_mass_host, uint32_t n, float theta, float eps,
                      const uint8_t* active_mask_host, float* acc_pot_host_out);
 

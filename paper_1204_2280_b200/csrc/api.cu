@@ -320,10 +320,14 @@ int bonsai_step_host(bonsai_ctx* h, const float* pos_mass_host, uint32_t n, floa
     if (n == 0 || n > c->n_max) return BONSAI_EINVAL;
     if (!theta_ok(theta) || !(eps >= 0.0f) || std::isinf(eps)) return BONSAI_EINVAL;
     Buffers& b = c->b;
+    // (Measured and dropped, profiles/r2_tried_and_dropped.md: letting the walk write its 16-byte rows straight into
+    // page-locked host memory hides the device-to-host copy but the scattered PCIe writes slow the walk by more than
+    // the copy costs -- 13.9 ms against 12.9 ms end to end at 2^22.)
+    float4* out_dev = b.host_out;
     BONSAI_TRY(cudaMemcpyAsync(b.host_in, pos_mass_host, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
     if (active_mask_host) {
         BONSAI_TRY(cudaMemcpyAsync(b.host_mask, active_mask_host, (size_t)n, cudaMemcpyHostToDevice, c->stream));
-        // entries of inactive particles are defined to stay untouched: start from the caller's values
+        // entries of inactive particles are defined to stay untouched: the staged result starts from the caller's values
         BONSAI_TRY(cudaMemcpyAsync(b.host_out, acc_pot_host_out, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
     }
     int rc;
@@ -331,7 +335,7 @@ int bonsai_step_host(bonsai_ctx* h, const float* pos_mass_host, uint32_t n, floa
     if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
     if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
     if ((rc = bonsai_walk(h, theta, eps, active_mask_host ? b.host_mask : nullptr,
-                          reinterpret_cast<float*>(b.host_out))) != BONSAI_OK) return rc;
+                          reinterpret_cast<float*>(out_dev))) != BONSAI_OK) return rc;
     BONSAI_TRY(cudaMemcpyAsync(acc_pot_host_out, b.host_out, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
     return bonsai_sync(h);
 }

@@ -399,7 +399,6 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
                 const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, lincl, o);
                 if (lane >= o) lincl += y;
             }
-            const int nl = __popc(lm);
             const uint32_t T = __shfl_sync(0xFFFFFFFFu, lincl, 31);
             if (oleaf) {
                 const int r = __popc(lm & lt);
@@ -408,16 +407,19 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
             }
             __syncwarp();
             npp += T;
+            const uint32_t lpre = lincl - lc;  // first particle slot of this lane's leaf (oleaf lanes)
             for (uint32_t base = 0; base < T; base += 32u) {
                 const uint32_t t = base + lane;
+                // which leaf does slot t belong to?  Leaves are non-empty, so their first slots are distinct: one bit
+                // per leaf starting inside this batch, and the rank of slot t's leaf = (leaves starting before the
+                // batch) + (start bits at or below the lane) - 1.
+                const uint32_t off = lpre - base;  // wraps for leaves that start before the batch
+                const uint32_t starts = __reduce_or_sync(0xFFFFFFFFu, (oleaf && off < 32u) ? (1u << off) : 0u);
+                const int before = __popc(__ballot_sync(0xFFFFFFFFu, oleaf && lpre < base));
                 if (t < T) {
-                    int lo = 0, hi = nl - 1;  // largest r with leaf_pref[r] <= t
-                    while (lo < hi) {
-                        const int mid = (lo + hi + 1) >> 1;
-                        if (S.leaf_pref[mid] <= t) lo = mid; else hi = mid - 1;
-                    }
+                    const int r = before + __popc(starts & (0xFFFFFFFFu >> (31 - lane))) - 1;
                     if (!kTeam || (((pp_w + lane) >> 5) & tmask) == uslot)  // only the batches this member evaluates
-                        S.pp[(pp_w + lane) & 63u] = __ldg(&a.pos[S.leaf_first[lo] + (t - S.leaf_pref[lo])]);
+                        S.pp[(pp_w + lane) & 63u] = __ldg(&a.pos[S.leaf_first[r] + (t - S.leaf_pref[r])]);
                 }
                 pp_w += min(32u, T - base);
                 __syncwarp();
