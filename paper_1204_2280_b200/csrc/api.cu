@@ -75,6 +75,7 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     }
     t.ghist = cv.take<uint32_t>((size_t)kSortPasses * kRadix);
     t.look = cv.take<unsigned long long>((size_t)kRadix * n_tiles);
+    t.long_start = cv.take<uint32_t>((size_t)n / 32 + 1);
     t.bbox_partial = cv.take<float>(6 * kBboxMaxBlocks);
     t.sorted_pos = cv.take<float4>(n);
     t.lcp = cv.take<int8_t>((size_t)n + 1);
@@ -176,7 +177,6 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.pos_mass = nullptr;
     c.sorted_buf = 1;
     c.perm = c.b.idx[0];
-    c.sort_epoch = 0;
     c.state = 0;
     c.groups_all_active = false;
     c.tree_n = 0;

@@ -13,9 +13,9 @@ constexpr uint32_t kNone = 0xFFFFFFFFu;
 constexpr uint32_t kLeafBit = 0x80000000u;
 
 // ---- radix sort geometry (sort.cu) -------------------------------------------------------------
-constexpr int kRadixBits = 10;             // one 30-bit key word = 3 digits -> 9 LSD passes for 90 bits
+constexpr int kRadixBits = 10;             // one 30-bit key word = 3 digits
 constexpr int kRadix = 1 << kRadixBits;
-constexpr int kSortPasses = 9;
+constexpr int kSortPasses = 6;              // mid and hi words; the lo word is settled by the tie kernels
 constexpr int kSortThreads = 512;
 constexpr int kSortBlocksPerSM = 2;
 constexpr int kLookBatch = 1;              // look-back entries in flight per digit
@@ -59,7 +59,7 @@ struct Control {
     uint32_t level_ticket;     // last-block-done counter of k_tree_scan_levels
     uint32_t sort_ticket;      // tile scheduler of k_sort_pass (reset by the tile that draws the last ticket)
     uint32_t diag_ticket;      // last-block-done counter of k_diagnostics
-    uint32_t sort_fallback;    // set by k_sort_ties when a run of equal (hi, mid) is too long: the guarded chain runs
+    uint32_t n_long_runs;      // runs of equal (hi, mid) longer than kTieRun found by k_sort_ties (k_sort_long_runs)
     uint32_t recover_ticket;   // last-block-done counter of k_recover
     uint32_t rebuild_flag;     // R30: decision of k_rebuild_decide for the current tick (1 = rebuild, 0 = refresh)
     uint32_t tree_fresh;       // R30: set by a build; the next recorded walk becomes the reference and clears it
@@ -70,6 +70,10 @@ struct Control {
     double ipp_last;             // R30: ... of the last recorded walk
     uint32_t n_rebuilds;         // R30: rebuilds decided on the device since bonsai_create
     uint32_t n_decisions;
+    uint32_t sort_epoch;         // tag base of the look-back entries of this build's sort passes (k_bbox advances it)
+    uint32_t look_wrap;          // the epoch wrapped: k_sort_gscan clears the look-back table
+    uint32_t long_ticket;        // run scheduler / last-warp-done counter of k_sort_long_runs
+    uint32_t long_done;
 };
 
 // A launch that only does its work when a device flag has a given value.  The flag is written by an earlier kernel
@@ -109,6 +113,7 @@ struct Buffers {
     uint32_t* idx[2];
     uint32_t* ghist;           // [kSortPasses][kRadix] global digit histograms -> exclusive bases
     unsigned long long* look;  // [n_tiles][kRadix] decoupled look-back table of k_sort_pass
+    uint32_t* long_start;      // [n / 32 + 1] first position of every long run of equal (hi, mid)
     float* bbox_partial;       // [blocks][6]
     float4* sorted_pos;
     // tree
@@ -150,7 +155,6 @@ struct Ctx {
     const float4* pos_mass;    // caller's particles (load order)
     int sorted_buf;            // which key[] holds the sorted keys (1 once k_reorder has run)
     uint32_t* perm;            // perm[i] = load index of the i-th sorted particle (one of b.idx[])
-    uint32_t sort_epoch;       // tag of the last k_sort_pass launch (30 bits, see sort.cu)
     int state;                 // 0 created, 1 loaded, 2 tree built, 3 multipoles done, 4 walked
     bool groups_all_active;    // the group list on the device is the all-active one
     uint32_t tree_n;           // particle count of the tree on the device (0 = none): bonsai_refresh_tree may reuse it

@@ -79,6 +79,15 @@ __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, ui
         ctl->side_f = (float)side;
         ctl->scale = (float)(1073741824.0 / side);
         ctl->bbox_ticket = 0;  // ready for the next step
+        // one epoch per sort pass of this build (kSortPasses of them); on wrap-around of the 30-bit tag the look-back
+        // table is cleared by k_sort_gscan before the first pass
+        uint32_t ep = ctl->sort_epoch + 8u;
+        ctl->look_wrap = 0u;
+        if (ep >= (1u << 30) - 16u) {
+            ep = 8u;
+            ctl->look_wrap = 1u;
+        }
+        ctl->sort_epoch = ep;
     }
 }
 
@@ -87,7 +96,7 @@ __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, ui
 //   t = x - lo;  u = t * (2^30 / side);  i = trunc(u) clamped to [0, 2^30 - 1].
 // Octal digit of level L (1..30) = 4 x_bit + 2 y_bit + z_bit at bit 30 - L; words hi/mid/lo hold levels
 // 1-10 / 11-20 / 21-30.  Grid-stride, 16 B in, 3 x 4 B out, all coalesced.  The same pass builds the
-// digit histograms of all nine sort passes in shared memory (a histogram does not depend on the order
+// digit histograms of all six sort passes in shared memory (a histogram does not depend on the order
 // of the keys, so the sort never has to count again).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t spread10(uint32_t v) {  // 10 bits -> every third bit of 30
@@ -139,8 +148,8 @@ __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict_
             khi[i] = w[2];
         }
 #pragma unroll
-        for (int p = 0; p < kSortPasses; ++p) {
-            const uint32_t d = (w[p / 3] >> (kRadixBits * (p % 3))) & (kRadix - 1);
+        for (int p = 0; p < kSortPasses; ++p) {  // pass p sorts digit p % 3 of word 1 + p / 3 (mid, then hi)
+            const uint32_t d = (w[1 + p / 3] >> (kRadixBits * (p % 3))) & (kRadix - 1);
             // a warp whose 32 keys share the digit (the leading digits of clustered or pre-sorted input)
             // adds once instead of serialising 32 same-address atomics
             const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, d, 0);
@@ -158,13 +167,17 @@ __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict_
 
 // exclusive scan of each pass's histogram: ghist[p][d] <- sum_{d' < d} ghist[p][d'].  One block per pass.
 __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ ghist, Control* __restrict__ ctl,
+                                                       unsigned long long* __restrict__ look, size_t look_entries,
                                                        const Gate gate) {
     __shared__ uint32_t wsum[kRadix / 32];
     if (gate_closed(gate)) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
-        ctl->sort_fallback = 0;
+        ctl->n_long_runs = 0;
         ctl->tree_fresh = 1;  // R30: a new tree is being built; the next recorded walk is its reference
     }
+    if (ctl->look_wrap != 0u)  // the epoch tag wrapped (k_bbox): forget every stale entry of the look-back table
+        for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < look_entries; k += (size_t)gridDim.x * blockDim.x)
+            look[k] = 0ull;
     uint32_t* h = ghist + blockIdx.x * kRadix;
     uint32_t v = h[threadIdx.x];
     uint32_t x = v;
@@ -195,10 +208,10 @@ __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ gh
 // 30-bit word, index) PAIRS: a pass reads 8 B and writes 8 B per particle.  When the passes of one word are
 // done the next word is fetched through the index (gather from the load-order key arrays); the sorted
 // 90-bit keys are re-derived from the reordered positions in k_reorder (a key is a pure function of the
-// position and the root cube).  The sort proper runs SIX passes, over the mid and hi words: the lo word
-// (levels 21-30) almost never decides the order, and k_sort_ties repairs the runs of equal (hi, mid)
-// after the reorder; the full nine-pass chain (lo word first) stays enqueued behind a device flag for
-// inputs with long runs (see stage_sort_ties).
+// position and the root cube).  The sort runs SIX passes, over the mid and hi words: the lo word
+// (levels 21-30) almost never decides the order; the runs of equal (hi, mid) are put in order after the
+// reorder, short ones in place by k_sort_ties, long ones (coincident particles, clumps far smaller than
+// 2^-20 of the box) by k_sort_long_runs (see stage_sort_ties).
 //
 // One kernel per pass, single sweep with decoupled look-back:
 //   * tiles of kSortTile pairs are handed out by an atomic ticket, so a tile's predecessors have
@@ -208,7 +221,9 @@ __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ gh
 //   * each tile publishes, per digit, first its own count (AGGREGATE) and, after summing its
 //     predecessors' entries back to the nearest INCLUSIVE one, its inclusive prefix; an entry is one
 //     64-bit word {epoch : 30, flag : 2, value : 32}, the epoch (one per pass launch) makes stale
-//     entries of earlier passes read as "not yet written", so the table is never cleared;
+//     entries of earlier passes read as "not yet written", so the table is never cleared; the epoch
+//     lives on the device (Control::sort_epoch, advanced by k_bbox once per build) so that a captured
+//     CUDA graph of the step can be replayed;
 //   * the digit's global base comes from the all-pass histogram k_keys built;
 //   * pairs are first permuted into tile-sorted order in shared memory (aliasing the counters), so
 //     the global stores are runs of consecutive addresses per digit.
@@ -222,9 +237,9 @@ struct SortPass {
     const uint32_t* gbase;     // [kRadix] exclusive digit bases of this pass
     unsigned long long* look;  // [n_tiles][kRadix]
     uint32_t* ticket;
-    const uint32_t* guard;     // nullptr, or a device flag: the pass only runs when it is non-zero (fallback chain)
-    Gate gate;                 // and only when this gate is open (R30)
-    uint32_t n, n_tiles, epoch;
+    const Control* ctl;
+    Gate gate;                 // the pass only runs when this gate is open (R30)
+    uint32_t n, n_tiles, pass; // pass = 0 .. kSortPasses - 1: epoch of the launch = ctl->sort_epoch + pass
     int shift;
 };
 
@@ -257,7 +272,7 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
     __shared__ uint32_t s_wsum[kWarps];
     const int tid = threadIdx.x, l = tid & 31, w = tid >> 5;
     if (gate_closed(a.gate)) return;
-    if (a.guard != nullptr && __ldcg(a.guard) == 0u) return;  // uniform over the grid: the flag was set before the launch
+    const uint32_t epoch = __ldcg(&a.ctl->sort_epoch) + a.pass;
 
     if (tid == 0) {
         const uint32_t t = atomicAdd(a.ticket, 1u);
@@ -337,7 +352,7 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
     unsigned long long* my_look = a.look + (size_t)tile * kRadix + d0;
     const uint32_t first_flag = (tile == 0) ? kFlagIncl : kFlagAgg;
 #pragma unroll
-    for (int q = 0; q < kDig; ++q) look_store(my_look + q, look_pack(a.epoch, first_flag, tot[q]));
+    for (int q = 0; q < kDig; ++q) look_store(my_look + q, look_pack(epoch, first_flag, tot[q]));
     // block-wide exclusive scan of the digit totals -> first tile-sorted slot of each digit
     uint32_t x = 0;
 #pragma unroll
@@ -397,7 +412,7 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
         uint32_t pending = (1u << kDig) - 1u;
 #pragma unroll
         for (int q = 0; q < kDig; ++q) j[q] = tile - 1;
-        const uint32_t want = a.epoch;
+        const uint32_t want = epoch;
         // kLookBatch predecessors per digit are fetched together and consumed nearest-first: when a whole wave of
         // tiles publishes its aggregates at the same moment, the inclusive prefixes ripple forward one L2 round
         // trip per kLookBatch tiles instead of one per tile.
@@ -429,7 +444,7 @@ __global__ void __launch_bounds__(kSortThreads, kSortBlocksPerSM) k_sort_pass(co
             if (missed) __nanosleep(kLookSleepNs);     // keeps a waiting wave from flooding L2 with re-reads
         }
 #pragma unroll
-        for (int q = 0; q < kDig; ++q) look_store(my_look + q, look_pack(a.epoch, kFlagIncl, excl[q] + tot[q]));
+        for (int q = 0; q < kDig; ++q) look_store(my_look + q, look_pack(epoch, kFlagIncl, excl[q] + tot[q]));
     }
 #pragma unroll
     for (int q = 0; q < kDig; ++q) {
@@ -459,9 +474,8 @@ __global__ void __launch_bounds__(256) k_reorder(const float4* __restrict__ pos,
                                                  uint32_t n, const Control* __restrict__ ctl,
                                                  float4* __restrict__ sorted_pos, uint32_t* __restrict__ khi,
                                                  uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
-                                                 const uint32_t* __restrict__ guard, const Gate gate) {
+                                                 const Gate gate) {
     if (gate_closed(gate)) return;
-    if (guard != nullptr && __ldcg(guard) == 0u) return;
     const float lox = ctl->lo[0], loy = ctl->lo[1], loz = ctl->lo[2], scale = ctl->scale;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const float4 p = __ldg(&pos[__ldg(&perm[i])]);
@@ -497,18 +511,19 @@ cudaError_t stage_keys(Ctx* c) {
 // Ties of the two-word sort.  After the six passes over the mid and hi words the particles are ordered by their
 // first 20 octal digits and, inside a run of equal digits, by load index (LSD passes are stable).  Such runs are
 // cells of side 2^-20 of the root cube: with fp32 coordinates they hold one particle almost always.  The thread
-// at the head of a run orders it by (lo word, load index) with an insertion sort over perm, sorted_pos and the lo
-// keys; a run longer than kTieRun raises the fallback flag instead and the guarded nine-pass chain redoes the sort.
+// at the head of a run of up to kTieRun particles orders it by (lo word, load index) with an insertion sort over
+// perm, sorted_pos and the lo keys; the start of a longer run is appended to a device list that k_sort_long_runs
+// works off.
 constexpr uint32_t kTieRun = 32;
 
 __device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, const uint32_t* __restrict__ khi,
                                           const uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
                                           uint32_t* __restrict__ perm, float4* __restrict__ sorted_pos, uint32_t n,
-                                          Control* __restrict__ ctl) {
+                                          Control* __restrict__ ctl, uint32_t* __restrict__ long_start) {
     uint32_t len = 2;
     while (i + len < n && len <= kTieRun && khi[i + len] == h && kmid[i + len] == m) ++len;
     if (len > kTieRun) {
-        ctl->sort_fallback = 1;
+        long_start[atomicAdd(&ctl->n_long_runs, 1u)] = i;  // at most n / (kTieRun + 1) such runs
         return;
     }
     for (uint32_t k = 1; k < len; ++k) {  // stable insertion sort by lo: equal lo keep their ascending load index
@@ -532,7 +547,7 @@ __device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, co
 __global__ void __launch_bounds__(256) k_sort_ties(const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
                                                    uint32_t* __restrict__ klo, uint32_t* __restrict__ perm,
                                                    float4* __restrict__ sorted_pos, uint32_t n, Control* __restrict__ ctl,
-                                                   const Gate gate) {
+                                                   uint32_t* __restrict__ long_start, const Gate gate) {
     if (gate_closed(gate)) return;
     const uint32_t i0 = 4u * (blockIdx.x * blockDim.x + threadIdx.x);
     if (i0 >= n) return;
@@ -557,7 +572,123 @@ __global__ void __launch_bounds__(256) k_sort_ties(const uint32_t* __restrict__ 
         if (h[k] == 0xFFFFFFFFu) break;  // past the end (key words have 30 bits)
         const bool ties_next = (h[k + 1] == h[k]) && (m[k + 1] == m[k]);
         const bool ties_prev = (h[k - 1] == h[k]) && (m[k - 1] == m[k]);
-        if (ties_next && !ties_prev) sort_tie_run(i0 + k - 1, h[k], m[k], khi, kmid, klo, perm, sorted_pos, n, ctl);
+        if (ties_next && !ties_prev) sort_tie_run(i0 + k - 1, h[k], m[k], khi, kmid, klo, perm, sorted_pos, n, ctl, long_start);
+    }
+}
+
+// Long runs of equal (hi, mid): one WARP per run (runs are taken from the list by an atomic ticket) sorts the run
+// by (lo word, position in the run) -- a stable LSD radix sort over the 30 bits of the lo word, four passes of 8-bit
+// digits on (lo, local index) pairs in scratch arrays, then one gather of perm, sorted_pos and the lo keys through the
+// resulting order.  Positions in a run ascend with the load index (the six passes are stable), so this is exactly
+// the order (key, load index) of R5.  The launch returns at once when the list is empty (every Plummer / merger
+// workload); a degenerate input -- all particles coincident, or inside one cell of side 2^-20 -- costs this kernel a
+// few milliseconds instead of costing every step a nine-pass fallback chain of empty launches.
+struct LongRunScratch {
+    uint32_t *key_a, *key_b, *idx_a, *idx_b;  // [n] each, indexed by global position: runs are disjoint
+    uint32_t *perm_tmp, *lo_tmp;
+    float4* pos_tmp;
+};
+
+constexpr int kLongWarps = 4;
+
+__global__ void __launch_bounds__(kLongWarps * 32) k_sort_long_runs(const uint32_t* __restrict__ khi,
+                                                                    const uint32_t* __restrict__ kmid,
+                                                                    uint32_t* __restrict__ klo, uint32_t* __restrict__ perm,
+                                                                    float4* __restrict__ sorted_pos, uint32_t n,
+                                                                    Control* __restrict__ ctl,
+                                                                    const uint32_t* __restrict__ long_start,
+                                                                    LongRunScratch sc, const Gate gate) {
+    __shared__ uint32_t s_hist[kLongWarps][256];
+    if (gate_closed(gate)) return;
+    const uint32_t n_runs = __ldcg(&ctl->n_long_runs);
+    if (n_runs == 0u) return;
+    const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t lt = (1u << l) - 1u;
+    uint32_t* hist = s_hist[w];
+    for (;;) {
+        uint32_t r = 0;
+        if (l == 0) r = atomicAdd(&ctl->long_ticket, 1u);
+        r = __shfl_sync(0xFFFFFFFFu, r, 0);
+        if (r >= n_runs) break;
+        const uint32_t s0 = __ldcg(&long_start[r]);
+        const uint32_t h = khi[s0], m = kmid[s0];
+        // length of the run: first position that leaves it
+        uint32_t len = 0;
+        for (uint32_t base = s0;; base += 32u) {
+            const uint32_t i = base + l;
+            const bool in = i < n && khi[i] == h && kmid[i] == m;
+            const uint32_t out = ~__ballot_sync(0xFFFFFFFFu, in);
+            if (out) { len = base - s0 + (uint32_t)(__ffs(out) - 1); break; }
+        }
+        uint32_t *ka = sc.key_a + s0, *kb = sc.key_b + s0, *ia = sc.idx_a + s0, *ib = sc.idx_b + s0;
+        for (uint32_t k = l; k < len; k += 32u) { ka[k] = klo[s0 + k]; ia[k] = k; }
+        __syncwarp();
+        for (int shift = 0; shift < 30; shift += 8) {
+            for (int d = l; d < 256; d += 32) hist[d] = 0u;
+            __syncwarp();
+            for (uint32_t k = l; k < len; k += 32u) atomicAdd(&hist[(ka[k] >> shift) & 255u], 1u);
+            __syncwarp();
+            // exclusive scan of the 256 counts: 8 per lane, then across lanes
+            uint32_t v[8], sum = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { v[q] = hist[8 * l + q]; sum += v[q]; }
+            uint32_t incl = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                if (l >= o) incl += y;
+            }
+            uint32_t run = incl - sum;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { hist[8 * l + q] = run; run += v[q]; }
+            __syncwarp();
+            // stable scatter, 32 elements at a time in order: equal digits keep their order (lane order inside a
+            // chunk, chunk order through the running offsets)
+            for (uint32_t base = 0; base < len; base += 32u) {
+                const uint32_t k = base + l;
+                const bool valid = k < len;
+                const uint32_t key = valid ? ka[k] : 0u;
+                const uint32_t d = valid ? ((key >> shift) & 255u) : 256u + (uint32_t)l;  // invalid lanes match nobody
+                const uint32_t peers = __match_any_sync(0xFFFFFFFFu, d);
+                uint32_t off = 0;
+                if (valid) off = hist[d];
+                __syncwarp();
+                if (valid) {
+                    const uint32_t dst = off + (uint32_t)__popc(peers & lt);
+                    kb[dst] = key;
+                    ib[dst] = ia[k];
+                    if ((peers >> l) <= 1u) hist[d] = off + (uint32_t)__popc(peers);  // the highest peer advances the offset
+                }
+                __syncwarp();
+            }
+            uint32_t* t = ka; ka = kb; kb = t;
+            t = ia; ia = ib; ib = t;
+            __threadfence_block();
+            __syncwarp();
+        }
+        // ia[k] = position (in the run) of the particle that belongs at k
+        for (uint32_t k = l; k < len; k += 32u) {
+            sc.perm_tmp[s0 + k] = perm[s0 + k];
+            sc.lo_tmp[s0 + k] = klo[s0 + k];
+            sc.pos_tmp[s0 + k] = sorted_pos[s0 + k];
+        }
+        __threadfence_block();
+        __syncwarp();
+        for (uint32_t k = l; k < len; k += 32u) {
+            const uint32_t src = s0 + ia[k];
+            perm[s0 + k] = sc.perm_tmp[src];
+            klo[s0 + k] = sc.lo_tmp[src];
+            sorted_pos[s0 + k] = sc.pos_tmp[src];
+        }
+        __syncwarp();
+    }
+    // the last warp to leave resets the ticket for the next build (n_long_runs is reset by k_sort_gscan)
+    if (l == 0) {
+        __threadfence();
+        if (atomicAdd(&ctl->long_done, 1u) == gridDim.x * kLongWarps - 1u) {
+            ctl->long_done = 0u;
+            ctl->long_ticket = 0u;
+        }
     }
 }
 
@@ -572,81 +703,63 @@ cudaError_t sort_prepare(Ctx* c) {
     return e;
 }
 
-// Passes first_pass .. 8 of the LSD sort (pass p: word 2 - p / 3 = lo, mid, hi; digit p % 3), starting from the
-// identity permutation.  The first pass writes pair buffer first_out, every later pass flips; with first_out chosen
-// by the callers below both chains leave the permutation in idx[0].
-static cudaError_t sort_chain(Ctx* c, int first_pass, int first_out, const uint32_t* guard) {
+// The sort: six LSD passes over the mid and hi words (pass p: word mid, hi = p / 3; digit p % 3), starting from the
+// identity permutation; the outputs alternate pair buffers 1, 0, 1, 0, 1, 0, which leaves the permutation in idx[0].
+cudaError_t stage_sort(Ctx* c) {
     Buffers& b = c->b;
-    const size_t smem = kSortSmem;
-    cudaError_t e = cudaSuccess;
+    const size_t look_entries = (size_t)div_up(c->n_max, kSortTile) * kRadix;
+    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist, b.ctl, b.look, look_entries, c->gate);
+    c->launches += 1;
+    c->perm = b.idx[0];
     SortPass a;
     a.n = c->n;
     a.n_tiles = div_up(c->n, kSortTile);
     a.look = b.look;
     a.ticket = &b.ctl->sort_ticket;
-    a.guard = guard;
+    a.ctl = b.ctl;
     a.gate = c->gate;
-    int cur = first_out ^ 1;
-    for (int p = first_pass; p < kSortPasses; ++p) {
-        if (c->sort_epoch >= (1u << 30) - 1) {  // 30-bit epoch about to wrap: forget every stale entry
-            e = cudaMemsetAsync(b.look, 0, sizeof(unsigned long long) * (size_t)div_up(c->n_max, kSortTile) * kRadix, c->stream);
-            if (e != cudaSuccess) return e;
-            c->sort_epoch = 0;
-        }
-        a.epoch = ++c->sort_epoch;
+    int cur = 0;
+    for (int p = 0; p < kSortPasses; ++p) {
+        a.pass = (uint32_t)p;
         a.shift = kRadixBits * (p % 3);
         a.gbase = b.ghist + p * kRadix;
-        a.src_word = b.key[0][2 - p / 3];  // load-order word of this phase: lo, mid, hi
+        a.src_word = b.key[0][1 - p / 3];  // load-order word of this phase: mid, then hi
         const int out = cur ^ 1;
         a.key_in = b.pair_key[cur];
         a.idx_in = b.idx[cur];
         a.key_out = (p == kSortPasses - 1) ? nullptr : b.pair_key[out];
         a.idx_out = b.idx[out];
-        if (p == first_pass) k_sort_pass<0><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
-        else if (p % 3 == 0) k_sort_pass<2><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
-        else k_sort_pass<1><<<a.n_tiles, kSortThreads, smem, c->stream>>>(a);
+        if (p == 0) k_sort_pass<0><<<a.n_tiles, kSortThreads, kSortSmem, c->stream>>>(a);
+        else if (p % 3 == 0) k_sort_pass<2><<<a.n_tiles, kSortThreads, kSortSmem, c->stream>>>(a);
+        else k_sort_pass<1><<<a.n_tiles, kSortThreads, kSortSmem, c->stream>>>(a);
         c->launches += 1;
         cur = out;
     }
     return (cur == 0) ? cudaGetLastError() : cudaErrorUnknown;
 }
 
-// The sort proper: six passes over the mid and hi words (the lo word almost never decides the order, see k_sort_ties).
-cudaError_t stage_sort(Ctx* c) {
-    Buffers& b = c->b;
-    k_sort_gscan<<<kSortPasses, kRadix, 0, c->stream>>>(b.ghist, b.ctl, c->gate);
-    c->launches += 1;
-    c->perm = b.idx[0];
-    return sort_chain(c, 3, 1, nullptr);  // outputs 1, 0, 1, 0, 1, 0
-}
-
-static void launch_reorder(Ctx* c, bool write_keys, const uint32_t* guard) {
-    Buffers& b = c->b;
-    // the guarded instance normally returns at once: keep its grid small
-    const uint32_t blocks = guard ? (uint32_t)c->num_sms * 8u : div_up(c->n, 256);
-    k_reorder<<<blocks, 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos,
-                                             write_keys ? b.key[1][0] : nullptr, b.key[1][1], b.key[1][2], guard, c->gate);
-    c->launches += 1;
-}
-
 cudaError_t stage_reorder(Ctx* c, bool write_keys) {
-    launch_reorder(c, write_keys, nullptr);
+    Buffers& b = c->b;
+    k_reorder<<<div_up(c->n, 256), 256, 0, c->stream>>>(c->pos_mass, c->perm, c->n, b.ctl, b.sorted_pos,
+                                                        write_keys ? b.key[1][0] : nullptr, b.key[1][1], b.key[1][2], c->gate);
+    c->launches += 1;
     c->sorted_buf = 1;
     return cudaGetLastError();
 }
 
-// After the reorder of a fresh sort: order the (rare) runs of equal (hi, mid) by their lo word, and keep the full
-// nine-pass chain plus a second reorder enqueued behind the fallback flag for inputs with long runs (coincident
-// particles, clusters far smaller than 2^-20 of the box).  The guarded launches return at once in the normal case.
+// After the reorder of a fresh sort: put the (rare) runs of equal (hi, mid) in order of their lo word -- short runs in
+// place, long ones (coincident particles, clumps far smaller than 2^-20 of the box) by k_sort_long_runs, which
+// returns at once when there are none.  Scratch of the long-run sort: the pair buffers and the load-order key words
+// (dead after the passes) and the fp64 moment array (not yet written).
 cudaError_t stage_sort_ties(Ctx* c) {
     Buffers& b = c->b;
     k_sort_ties<<<div_up(div_up(c->n, 4), 256), 256, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
-                                                          b.ctl, c->gate);
-    c->launches += 1;
-    const uint32_t* guard = &b.ctl->sort_fallback;
-    cudaError_t e = sort_chain(c, 0, 0, guard);  // outputs 0, 1, 0, 1, 0, 1, 0, 1, 0
-    if (e != cudaSuccess) return e;
-    launch_reorder(c, true, guard);
+                                                          b.ctl, b.long_start, c->gate);
+    LongRunScratch sc{b.pair_key[0], b.pair_key[1], b.idx[1], b.key[0][0], b.key[0][1], b.key[0][2],
+                      reinterpret_cast<float4*>(b.c_mom)};
+    k_sort_long_runs<<<c->num_sms, kLongWarps * 32, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
+                                                                 b.ctl, b.long_start, sc, c->gate);
+    c->launches += 2;
     return cudaGetLastError();
 }
 

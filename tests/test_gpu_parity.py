@@ -309,13 +309,13 @@ def test_duplicate_positions_and_deep_chain():
     check_walk(b, out, ref, count_frac=0.98, eps=0.01, pm=pm)
 
 
-@pytest.mark.parametrize("clump_sizes", [(2, 3, 5, 17, 32), (33, 40, 200), (2, 31, 32, 33)])
+@pytest.mark.parametrize("clump_sizes", [(2, 3, 5, 17, 32), (33, 40, 200), (2, 31, 32, 33), (3000, 700, 64, 65)])
 def test_sort_ties_below_the_20th_level(clump_sizes):
     """The sort orders by the mid and hi key words and repairs runs of equal (hi, mid) afterwards (sort.cu): clumps
     far smaller than 2^-20 of the root cube with DISTINCT positions inside exercise the in-place repair (runs
-    <= 32) and the guarded nine-pass fallback (longer runs).  The permutation must still be the oracle's."""
+    <= 32) and the long-run radix sort (longer runs).  The permutation must still be the oracle's."""
     rng = np.random.default_rng(sum(clump_sizes))
-    n = 6000
+    n = 6000 + sum(clump_sizes)
     pm = W.plummer(n)
     pm[0, :3] = (900.0, -700.0, 800.0)                       # a far particle: root cube side 2048, 2^-20 side = 2e-3
     at = 100
@@ -349,15 +349,17 @@ def test_merger_workload(mode):
     check_walk(b, out, ref)
 
 
-def test_all_particles_coincident():
-    pm = np.zeros((100, 4), np.float32)
+@pytest.mark.parametrize("n", [100, 20_000])
+def test_all_particles_coincident(n):
+    pm = np.zeros((n, 4), np.float32)
     pm[:, :3] = (1.0, 2.0, 3.0)
-    pm[:, 3] = 0.01
+    pm[:, 3] = 1.0 / n
     ref = O.build(pm)
-    b = Bonsai(100)
-    b.load(_dev(pm)); b.build_tree(); b.compute_multipoles(); b.sync()
-    check_structure(b, ref)
-    check_groups(b, ref)
+    b = Bonsai(n)
+    for _ in range(2):  # twice: the long-run scheduler state must be reset between builds
+        b.load(_dev(pm)); b.build_tree(); b.compute_multipoles(); b.sync()
+        check_structure(b, ref)
+        check_groups(b, ref)
 
 
 def test_reuse_context_smaller_n_and_repeat():
