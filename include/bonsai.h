@@ -66,6 +66,8 @@ typedef struct {
                             of the cell's particles, l_t = its longest side, centre = its midpoint (R28)         */
     uint32_t order;      /* [2] multipole order of a particle-cell interaction: 2 = monopole + quadrupole (R8),
                             1 = monopole only (R29); 0 = default                                                */
+    uint32_t no_graph;   /* [0] 1 = bonsai_step / bonsai_leapfrog_step enqueue their kernels one by one; 0 = they
+                            are captured as a CUDA graph and replayed while buffers and parameters repeat         */
     float rebuild_factor;/* [1.25] bonsai_block_tick(rebuild = -1) rebuilds the tree when the interactions per
                             walked sink of the last walk exceed rebuild_factor x those of the first walk after the
                             last build (R30); >= 1                                                       */
@@ -117,6 +119,16 @@ int bonsai_compute_multipoles(bonsai_ctx* ctx);
  *                    particles are written.
  * Per-particle interaction counts are kept for bonsai_get_counts().  EINVAL, ESTATE before multipoles. */
 int bonsai_walk(bonsai_ctx* ctx, float theta, float eps, const uint8_t* active_mask_dev, float* acc_pot_dev_out);
+
+/* One full force step = bonsai_load, bonsai_build_tree, bonsai_compute_multipoles, bonsai_walk (arguments as
+ * there), as ONE call.  Unless params.no_graph is set or stage timing is on, the sequence is captured as a CUDA graph
+ * the first time a combination (pos_mass_dev, n, theta, eps, active_mask_dev, acc_pot_dev_out) is seen -- on a stream
+ * the library owns, so the caller's stream may be the legacy default stream -- and replayed with one graph launch
+ * from then on (the four most recent combinations are kept): below ~10^5 particles a step is bound by launch gaps
+ * (P:L32).  The replay enqueues exactly the kernels of the staged calls; results are bit-identical.
+ * EINVAL / ESTATE / ECUDA as the staged calls. */
+int bonsai_step(bonsai_ctx* ctx, const float* pos_mass_dev, uint32_t n, float theta, float eps,
+                const uint8_t* active_mask_dev, float* acc_pot_dev_out);
 
 /* One full force step for a caller whose particles live in HOST memory (the end-to-end path of bench.py):
  * copies pos_mass_host (float4[n]; pinned memory recommended) to a staging buffer in the workspace, runs
@@ -283,8 +295,10 @@ int bonsai_get_rebuild_stats(bonsai_ctx* ctx, uint32_t* n_decisions, uint32_t* n
 int bonsai_set_timing(bonsai_ctx* ctx, int enable);
 int bonsai_get_stage_ms(bonsai_ctx* ctx, float out_ms[BONSAI_N_STAGES]);
 
-/* Number of kernel launches the library has enqueued since bonsai_create(). */
+/* Number of kernel launches the library has enqueued since bonsai_create() (kernels inside replayed graphs
+ * included), and how many calls were served by replaying a captured graph. */
 uint64_t bonsai_get_launch_count(bonsai_ctx* ctx);
+uint64_t bonsai_get_graph_replays(bonsai_ctx* ctx);
 
 /* Measurement support (not a step of the method): the FP32 throughput of the current CUDA device, measured with a
  * register-only loop of independent chains of the instruction the walk's interaction loops are made of --

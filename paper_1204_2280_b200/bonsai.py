@@ -31,14 +31,14 @@ SYMBOLS = (
     "bonsai_get_launch_count", "bonsai_strerror",
     "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
     "bonsai_timestep_rungs", "bonsai_active_mask", "bonsai_kick_rungs", "bonsai_block_tick",
-    "bonsai_measure_fp32_peak", "bonsai_get_rebuild_stats",
+    "bonsai_measure_fp32_peak", "bonsai_get_rebuild_stats", "bonsai_step", "bonsai_get_graph_replays",
 )
 
 
 class Params(C.Structure):
     _fields_ = [("nleaf", C.c_uint32), ("ncrit", C.c_uint32), ("group_mode", C.c_uint32),
                 ("cap_cells", C.c_uint32), ("group_cell", C.c_uint32), ("mac_mode", C.c_uint32),
-                ("order", C.c_uint32), ("rebuild_factor", C.c_float)]
+                ("order", C.c_uint32), ("no_graph", C.c_uint32), ("rebuild_factor", C.c_float)]
 
 
 class CellsView(C.Structure):
@@ -76,6 +76,9 @@ def lib() -> C.CDLL:
     L.bonsai_compute_multipoles.argtypes = [vp]
     L.bonsai_walk.argtypes = [vp, f32, f32, vp, vp]
     L.bonsai_step_host.argtypes = [vp, vp, u32, f32, f32, vp, vp]
+    L.bonsai_step.argtypes = [vp, vp, u32, f32, f32, vp, vp]
+    L.bonsai_get_graph_replays.argtypes = [vp]
+    L.bonsai_get_graph_replays.restype = C.c_uint64
     L.bonsai_destroy.argtypes = [vp]
     L.bonsai_destroy.restype = None
     L.bonsai_sync.argtypes = [vp]
@@ -132,7 +135,7 @@ def measure_fp32_peak(packed: bool = True, iters: int = 20000, stream: "torch.cu
 
 def workspace_bytes(n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
                     cap_cells: int = 0, group_cell: int = 0, mac_mode: int = 0, order: int = 2) -> int:
-    p = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order, 0.0)
+    p = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order, 0, 0.0)
     return int(lib().bonsai_workspace_bytes(n_max, C.byref(p)))
 
 
@@ -178,14 +181,15 @@ class Bonsai:
     def __init__(self, n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
                  cap_cells: int = 0, group_cell: int = 0, device: str | torch.device = "cuda:0",
                  stream: "torch.cuda.Stream | None" = None, mac_mode: int = 0, order: int = 2,
-                 rebuild_factor: float = 0.0):
+                 rebuild_factor: float = 0.0, use_graph: bool = True):
         if not torch.cuda.is_available():
             raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
         self.device = torch.device(device)
         self._L = lib()
         self.n_max = int(n_max)
         self.n = 0
-        self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order, rebuild_factor)
+        self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order, 0 if use_graph else 1,
+                             rebuild_factor)
         nbytes = int(self._L.bonsai_workspace_bytes(self.n_max, C.byref(self.params)))
         if nbytes == 0:
             raise BonsaiError(EINVAL, "bonsai_workspace_bytes")
@@ -241,11 +245,26 @@ class Bonsai:
         return out
 
     def step(self, pos_mass: torch.Tensor, theta: float, eps: float, active_mask=None, out=None) -> torch.Tensor:
-        """One full force step: load -> build_tree -> compute_multipoles -> walk (no host sync)."""
-        self.load(pos_mass)
-        self.build_tree()
-        self.compute_multipoles()
-        return self.walk(theta, eps, active_mask, out)
+        """bonsai_step: load -> build_tree -> compute_multipoles -> walk as one call (no host sync); replayed as a
+        CUDA graph while the same tensors and parameters come back (unless use_graph=False or timing is on)."""
+        assert pos_mass.is_cuda and pos_mass.dtype == torch.float32 and pos_mass.is_contiguous()
+        assert pos_mass.dim() == 2 and pos_mass.shape[1] == 4
+        n = pos_mass.shape[0]
+        if out is None:
+            with torch.cuda.stream(self.stream):
+                out = torch.zeros((n, 4), dtype=torch.float32, device=self.device)
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.shape == (n, 4)
+        mptr = None
+        if active_mask is not None:
+            assert active_mask.is_cuda and active_mask.dtype == torch.uint8 and active_mask.is_contiguous()
+            assert active_mask.numel() == n
+            mptr = active_mask.data_ptr()
+        with torch.cuda.device(self.device):
+            _check(self._L.bonsai_step(self._h, pos_mass.data_ptr(), n, float(theta), float(eps), mptr, out.data_ptr()),
+                   "bonsai_step")
+        self.n = n
+        self._keep = [pos_mass] + ([active_mask] if active_mask is not None else [])
+        return out
 
     def step_host(self, pos_mass_host: torch.Tensor, theta: float, eps: float,
                   active_mask_host: torch.Tensor | None = None, out_host: torch.Tensor | None = None) -> torch.Tensor:
@@ -395,6 +414,9 @@ class Bonsai:
 
     def launch_count(self) -> int:
         return int(self._L.bonsai_get_launch_count(self._h))
+
+    def graph_replays(self) -> int:
+        return int(self._L.bonsai_get_graph_replays(self._h))
 
     def interaction_totals(self) -> tuple[int, int]:
         a, b = C.c_uint64(0), C.c_uint64(0)

@@ -30,8 +30,9 @@ struct Carver {
 
 bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out) {
     bonsai_params p;
-    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0; p.mac_mode = 0; p.order = 2; p.rebuild_factor = 0.0f;
+    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0; p.mac_mode = 0; p.order = 2; p.rebuild_factor = 0.0f; p.no_graph = 0;
     if (in) {
+        p.no_graph = in->no_graph;
         p.rebuild_factor = in->rebuild_factor;
         p.mac_mode = in->mac_mode;
         if (in->order) p.order = in->order;
@@ -196,6 +197,9 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.device = dev;
     c.gate = Gate{nullptr, 0u};
     c.tree_auto = false;
+    c.capture_stream = nullptr;
+    c.graph_clock = c.graph_replays = 0;
+    for (int k = 0; k < kGraphSlots; ++k) c.graphs[k].valid = false;
     // kernel attributes and occupancy are per device: set for every context (idempotent), never behind a
     // process-wide flag
     if (walk_prepare(&c) != cudaSuccess || sort_prepare(&c) != cudaSuccess) {
@@ -313,6 +317,104 @@ int bonsai_walk(bonsai_ctx* h, float theta, float eps, const uint8_t* active_mas
     return BONSAI_OK;
 }
 
+
+}  // extern "C"
+
+// ---- captured sequences (GraphKey / GraphSlot, internal.cuh) ------------------------------------------------------------
+
+namespace {
+
+HostState host_state(const Ctx* c) {
+    return HostState{c->pos_mass, c->n, c->tree_n, c->state, c->sorted_buf, c->groups_all_active, c->tree_refreshed,
+                     c->tree_auto, c->perm};
+}
+
+void restore_host_state(Ctx* c, const HostState& s) {
+    c->pos_mass = s.pos_mass; c->n = s.n; c->tree_n = s.tree_n; c->state = s.state; c->sorted_buf = s.sorted_buf;
+    c->groups_all_active = s.groups_all_active; c->tree_refreshed = s.tree_refreshed; c->tree_auto = s.tree_auto;
+    c->perm = s.perm;
+}
+
+// Runs `enqueue` (a sequence of C-ABI calls on h) either directly on the caller's stream, or -- when graphs are
+// enabled and stage timing is off -- as a CUDA graph: captured on the library's own stream the first time this key
+// is seen, replayed on the caller's stream from then on.  A failed capture falls back to the direct path.
+template <class F>
+int run_sequence(bonsai_ctx* h, const GraphKey& key, F&& enqueue) {
+    Ctx* c = &h->c;
+    if (c->prm.no_graph || c->timing) return enqueue();
+    c->graph_clock += 1;
+    for (int k = 0; k < kGraphSlots; ++k) {
+        GraphSlot& g = c->graphs[k];
+        if (g.valid && g.key == key) {
+            if (cudaGraphLaunch(g.exec, c->stream) != cudaSuccess) return BONSAI_ECUDA;
+            restore_host_state(c, g.after);
+            c->launches += g.launches;
+            c->graph_replays += 1;
+            g.last_use = c->graph_clock;
+            return BONSAI_OK;
+        }
+    }
+    if (!c->capture_stream && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return enqueue();
+    }
+    const HostState before = host_state(c);
+    const uint64_t launches0 = c->launches;
+    cudaStream_t user = c->stream;
+    if (cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return enqueue();
+    }
+    c->stream = c->capture_stream;
+    const int rc = enqueue();
+    c->stream = user;
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(c->capture_stream, &graph);
+    cudaGraphExec_t exec = nullptr;
+    if (rc != BONSAI_OK || ce != cudaSuccess || graph == nullptr ||
+        cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        (void)cudaGetLastError();
+        restore_host_state(c, before);
+        c->launches = launches0;
+        if (rc != BONSAI_OK) return rc;  // an argument / state error: the same answer without a graph
+        return enqueue();
+    }
+    cudaGraphDestroy(graph);
+    int slot = 0;  // a free slot, else the least recently used
+    for (int k = 0; k < kGraphSlots; ++k) {
+        if (!c->graphs[k].valid) { slot = k; break; }
+        if (c->graphs[k].last_use < c->graphs[slot].last_use) slot = k;
+    }
+    GraphSlot& g = c->graphs[slot];
+    if (g.valid) cudaGraphExecDestroy(g.exec);
+    g.valid = true;
+    g.key = key;
+    g.exec = exec;
+    g.after = host_state(c);
+    g.launches = c->launches - launches0;
+    g.last_use = c->graph_clock;
+    if (cudaGraphLaunch(exec, c->stream) != cudaSuccess) return BONSAI_ECUDA;
+    return BONSAI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int bonsai_step(bonsai_ctx* h, const float* pos_mass_dev, uint32_t n, float theta, float eps,
+                const uint8_t* active_mask_dev, float* acc_pot_dev_out) {
+    if (!h || !pos_mass_dev || !acc_pot_dev_out) return BONSAI_EINVAL;
+    const GraphKey key{1, {pos_mass_dev, active_mask_dev, acc_pot_dev_out, nullptr}, n, {theta, eps, 0.0f}};
+    return run_sequence(h, key, [&]() -> int {
+        int rc;
+        if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
+        if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
+        if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
+        return bonsai_walk(h, theta, eps, active_mask_dev, acc_pot_dev_out);
+    });
+}
+
 int bonsai_step_host(bonsai_ctx* h, const float* pos_mass_host, uint32_t n, float theta, float eps,
                      const uint8_t* active_mask_host, float* acc_pot_host_out) {
     if (!h || !pos_mass_host || !acc_pot_host_out) return BONSAI_EINVAL;
@@ -331,11 +433,9 @@ int bonsai_step_host(bonsai_ctx* h, const float* pos_mass_host, uint32_t n, floa
         BONSAI_TRY(cudaMemcpyAsync(b.host_out, acc_pot_host_out, sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
     }
     int rc;
-    if ((rc = bonsai_load(h, reinterpret_cast<const float*>(b.host_in), n)) != BONSAI_OK) return rc;
-    if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
-    if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
-    if ((rc = bonsai_walk(h, theta, eps, active_mask_host ? b.host_mask : nullptr,
-                          reinterpret_cast<float*>(out_dev))) != BONSAI_OK) return rc;
+    if ((rc = bonsai_step(h, reinterpret_cast<const float*>(b.host_in), n, theta, eps,
+                          active_mask_host ? b.host_mask : nullptr, reinterpret_cast<float*>(out_dev))) != BONSAI_OK)
+        return rc;
     BONSAI_TRY(cudaMemcpyAsync(acc_pot_host_out, b.host_out, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
     return bonsai_sync(h);
 }
@@ -387,22 +487,25 @@ int bonsai_leapfrog_step(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, flo
     if (!theta_ok(theta) || !(eps >= 0.0f) || std::isinf(eps)) return BONSAI_EINVAL;
     Ctx* c = &h->c;
     const float half = 0.5f * dt;  // exact
-    {
-        StageTimer t(c, 8);
-        BONSAI_TRY(stage_kick_drift(c, reinterpret_cast<float4*>(pos_mass_dev), reinterpret_cast<float4*>(vel_dev),
-                                    reinterpret_cast<const float4*>(acc_pot_dev), n, half, dt));
-    }
-    int rc;
-    if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
-    if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
-    if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
-    if ((rc = bonsai_walk(h, theta, eps, nullptr, acc_pot_dev)) != BONSAI_OK) return rc;
-    {
-        StageTimer t(c, 8);
-        BONSAI_TRY(stage_kick(c, reinterpret_cast<float4*>(vel_dev), reinterpret_cast<const float4*>(acc_pot_dev), n, half,
-                              nullptr));
-    }
-    return BONSAI_OK;
+    const GraphKey key{2, {pos_mass_dev, vel_dev, acc_pot_dev, nullptr}, n, {theta, eps, dt}};
+    return run_sequence(h, key, [&]() -> int {
+        {
+            StageTimer t(c, 8);
+            BONSAI_TRY(stage_kick_drift(c, reinterpret_cast<float4*>(pos_mass_dev), reinterpret_cast<float4*>(vel_dev),
+                                        reinterpret_cast<const float4*>(acc_pot_dev), n, half, dt));
+        }
+        int rc;
+        if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
+        if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
+        if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
+        if ((rc = bonsai_walk(h, theta, eps, nullptr, acc_pot_dev)) != BONSAI_OK) return rc;
+        {
+            StageTimer t(c, 8);
+            BONSAI_TRY(stage_kick(c, reinterpret_cast<float4*>(vel_dev), reinterpret_cast<const float4*>(acc_pot_dev), n, half,
+                                  nullptr));
+        }
+        return BONSAI_OK;
+    });
 }
 
 // ---- block time-steps (R26, R27) --------------------------------------------------------------------------
@@ -478,6 +581,9 @@ int bonsai_block_tick(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, float*
 
 void bonsai_destroy(bonsai_ctx* h) {
     if (!h) return;
+    for (int k = 0; k < kGraphSlots; ++k)
+        if (h->c.graphs[k].valid) cudaGraphExecDestroy(h->c.graphs[k].exec);
+    if (h->c.capture_stream) cudaStreamDestroy(h->c.capture_stream);
     for (int s = 0; s < BONSAI_N_STAGES; ++s)
         for (int i = 0; i < kStageIntervals; ++i)
             for (int k = 0; k < 2; ++k)
@@ -625,6 +731,8 @@ int bonsai_get_stage_ms(bonsai_ctx* h, float out_ms[BONSAI_N_STAGES]) {
 }
 
 uint64_t bonsai_get_launch_count(bonsai_ctx* h) { return h ? h->c.launches : 0; }
+
+uint64_t bonsai_get_graph_replays(bonsai_ctx* h) { return h ? h->c.graph_replays : 0; }
 
 const char* bonsai_strerror(int code) {
     switch (code) {

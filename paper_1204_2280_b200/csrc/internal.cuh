@@ -146,6 +146,37 @@ struct Buffers {
     uint8_t* tick_mask;        // [n] active mask of bonsai_block_tick
 };
 
+// A whole call sequence (bonsai_step, bonsai_leapfrog_step) captured once as a CUDA graph and replayed while the
+// caller keeps passing the same buffers and parameters: one graph launch instead of ~27 kernel launches -- below
+// N ~ 10^5 the step is bound by launch gaps, not by the kernels ("the algorithms require more than 10^5
+// particles to saturate the GPU").  Nothing in a step depends on host-side values that change between replays
+// (grid sizes depend on n only; the sort's look-back epoch lives on the device).
+struct GraphKey {
+    int kind;                  // 1 = bonsai_step, 2 = bonsai_leapfrog_step
+    const void* ptr[4];
+    uint32_t n;
+    float f[3];
+    bool operator==(const GraphKey& o) const {
+        return kind == o.kind && ptr[0] == o.ptr[0] && ptr[1] == o.ptr[1] && ptr[2] == o.ptr[2] && ptr[3] == o.ptr[3] &&
+               n == o.n && f[0] == o.f[0] && f[1] == o.f[1] && f[2] == o.f[2];
+    }
+};
+struct HostState {            // what a captured sequence leaves behind in the Ctx (restored on replay)
+    const float4* pos_mass;
+    uint32_t n, tree_n;
+    int state, sorted_buf;
+    bool groups_all_active, tree_refreshed, tree_auto;
+    uint32_t* perm;
+};
+struct GraphSlot {
+    bool valid;
+    GraphKey key;
+    cudaGraphExec_t exec;
+    HostState after;
+    uint64_t launches, last_use;
+};
+constexpr int kGraphSlots = 4;
+
 struct Ctx {
     uint32_t n_max, n;
     bonsai_params prm;
@@ -165,6 +196,9 @@ struct Ctx {
     uint64_t launches;
     int num_sms;
     int device;                // the CUDA device the context was created on
+    cudaStream_t capture_stream;  // library-owned stream the sequences are captured on (any caller stream can replay)
+    GraphSlot graphs[kGraphSlots];
+    uint64_t graph_clock, graph_replays;
     Gate gate;                 // applied to every launch of the build chain (bbox .. tree) while it is set (R30)
     bool tree_auto;            // the tree on the device was rebuilt OR refreshed by a device-side decision (R30)
     int walk_blocks_per_sm[8]; // occupancy of the k_walk instances on this device (set in bonsai_create)

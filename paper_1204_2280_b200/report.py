@@ -132,6 +132,22 @@ def scaling(reps: int) -> dict:
         total = sum(st.values())
         rows[name] = {"n": n, "stage_ms": st, "step_ms": total, "particles_per_s": n / (total * 1e-3),
                       "walk_share": st["walk"] / total, "pp_per_particle": pp / n, "pc_per_particle": pc / n}
+        # the un-instrumented step: replayed CUDA graph (bonsai_step) against kernel-by-kernel launches
+        b.set_timing(False)
+        out = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+        for tag, bb in (("step_ms_graph", b), ("step_ms_no_graph", Bonsai(n, use_graph=False))):
+            for _ in range(3):
+                bb.step(pm, theta, eps, None, out)
+            bb.sync()
+            ms = []
+            for _ in range(max(reps, 5)):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(bb.stream)
+                bb.step(pm, theta, eps, None, out)
+                e1.record(bb.stream)
+                bb.sync()
+                ms.append(e0.elapsed_time(e1))
+            rows[name][tag] = float(np.median(ms))
         del b
     return rows
 

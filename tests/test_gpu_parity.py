@@ -405,6 +405,45 @@ def _nan_out(n):
     return torch.full((n, 4), float("nan"), dtype=torch.float32, device="cuda")
 
 
+def test_graph_replay_is_bit_identical_to_the_staged_calls():
+    """bonsai_step captures load / build / multipoles / walk as a CUDA graph and replays it while the same buffers and
+    parameters come back.  Replays must return bit for bit what the staged calls (no graph) return, for alternating
+    keys (with / without mask, two theta), for changed particle DATA in the same buffer, and the replay counter must
+    show that graphs were actually used."""
+    n = 30_000
+    pm = W.plummer(n)
+    mask = W.active_mask(pm, n // 10, "clustered")
+    d_pm, d_mask = _dev(pm), _dev(mask)
+    ref_b = Bonsai(n, use_graph=False)
+    b = Bonsai(n)                                          # graphs on, caller stream = the legacy default stream
+    out_a = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+    out_m = torch.full((n, 4), 7.0, dtype=torch.float32, device="cuda")
+    want = {}
+    for key, (theta, m) in {"a": (0.75, None), "b": (0.5, None), "m": (0.75, d_mask)}.items():
+        o = torch.full((n, 4), 7.0, dtype=torch.float32, device="cuda")
+        want[key] = ref_b.step(d_pm, theta, 0.01, m, o).cpu().numpy().copy()
+    for rep in range(3):
+        for key, (theta, m, o) in {"a": (0.75, None, out_a), "b": (0.5, None, out_a), "m": (0.75, d_mask, out_m)}.items():
+            got = b.step(d_pm, theta, 0.01, m, o).cpu().numpy()
+            assert np.array_equal(got.view(np.uint32), want[key].view(np.uint32)), (rep, key)
+    assert b.graph_replays() >= 6 and ref_b.graph_replays() == 0
+    # the graph reads the buffer, not a snapshot: new positions in the same tensor, same graph
+    pm2 = W.plummer(n, seed=99)
+    d_pm.copy_(torch.from_numpy(pm2))
+    got = b.step(d_pm, 0.75, 0.01, None, out_a).cpu().numpy()
+    b.sync()
+    ref = O.full_step(pm2, 0.75, 0.01)
+    check_structure(b, ref)
+    check_groups(b, ref)
+    check_walk(b, got, ref, tag="graph replay, new data")
+    # stage timing switches the graph off (events are not captured) and still gives the same result
+    b.set_timing(True)
+    r0 = b.graph_replays()
+    got2 = b.step(d_pm, 0.75, 0.01, None, out_a).cpu().numpy()
+    assert b.graph_replays() == r0 and np.array_equal(got2.view(np.uint32), got.view(np.uint32))
+    assert b.stage_ms()["walk"] > 0
+
+
 def test_status_is_cleared_by_the_next_build():
     """A capacity overflow is reported by the bonsai_sync of that step and must not poison the context: the next
     bonsai_build_tree clears the sticky status and repairs the arrival counters the overflow left behind."""
