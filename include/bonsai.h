@@ -307,6 +307,12 @@ uint64_t bonsai_get_graph_replays(bonsai_ctx* ctx);
  * Blocks until done.  bench.py reports the walk's flop/s against this next to the derived peak.  EINVAL / ECUDA. */
 int bonsai_measure_fp32_peak(void* cuda_stream, int packed, int iters, double* tflops_out);
 
+/* Measurement support: issue cost of other instruction classes next to packed FMAs.  Every round of a warp is
+ * eight FFMA2 plus: kind 0 nothing, 1 eight LOP3 (integer ALU), 2 four LDS.128, 3 two MUFU.RSQ.  Writes the scheduler
+ * cycles one round costs (at the device's nominal clock; 16 with nothing added, since an FFMA2 holds the FP32 pipe
+ * for two cycles).  What exceeds 16 is what the added instructions cost the walk's interaction loops. */
+int bonsai_measure_issue_mix(void* cuda_stream, int kind, int iters, double* cycles_per_round_out);
+
 const char* bonsai_strerror(int code);
 
 #ifdef __cplusplus

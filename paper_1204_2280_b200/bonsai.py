@@ -32,6 +32,7 @@ SYMBOLS = (
     "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
     "bonsai_timestep_rungs", "bonsai_active_mask", "bonsai_kick_rungs", "bonsai_block_tick",
     "bonsai_measure_fp32_peak", "bonsai_get_rebuild_stats", "bonsai_step", "bonsai_get_graph_replays",
+    "bonsai_measure_issue_mix",
 )
 
 
@@ -105,6 +106,7 @@ def lib() -> C.CDLL:
     L.bonsai_leapfrog_step.argtypes = [vp, vp, vp, vp, u32, f32, f32, f32]
     L.bonsai_diagnostics.argtypes = [vp, vp, vp, vp, u32, vp]
     L.bonsai_get_rebuild_stats.argtypes = [vp, C.POINTER(u32), C.POINTER(u32), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.bonsai_measure_issue_mix.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
     L.bonsai_measure_fp32_peak.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
     L.bonsai_strerror.argtypes = [C.c_int]
     L.bonsai_strerror.restype = C.c_char_p
@@ -131,6 +133,19 @@ def measure_fp32_peak(packed: bool = True, iters: int = 20000, stream: "torch.cu
     st = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     _check(lib().bonsai_measure_fp32_peak(st, int(bool(packed)), int(iters), C.byref(out)), "bonsai_measure_fp32_peak")
     return float(out.value)
+
+
+def measure_issue_mix(iters: int = 20000) -> dict:
+    """bonsai_measure_issue_mix for the four kinds: scheduler cycles per round of 8 FFMA2 (+ other instructions)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
+    out = {}
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    for kind, name in enumerate(("ffma2_x8", "ffma2_x8+lop3_x8", "ffma2_x8+lds128_x4", "ffma2_x8+mufu_x2")):
+        v = C.c_double(0.0)
+        _check(lib().bonsai_measure_issue_mix(st, kind, int(iters), C.byref(v)), "bonsai_measure_issue_mix")
+        out[name] = float(v.value)
+    return out
 
 
 def workspace_bytes(n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,

@@ -208,15 +208,24 @@ def mac_variants(reps: int) -> dict:
             "variants": rows}
 
 
+def issue_mix(reps: int) -> dict:
+    """Microbenchmarks behind the walk's roofline argument: measured FP32 peak with FFMA2 and
+    FFMA, and what integer-ALU, shared-memory and MUFU instructions cost next to packed FMAs."""
+    from .bonsai import measure_fp32_peak, measure_issue_mix
+    del reps
+    return {"fp32_peak_tflops": {"ffma2": measure_fp32_peak(True, 40000), "ffma": measure_fp32_peak(False, 40000)},
+            "scheduler_cycles_per_round": measure_issue_mix(40000)}
+
+
 def main() -> None:
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--reps", type=int, default=5)
-    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling", "merger", "mac"), default=None)
+    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling", "merger", "mac", "issue_mix"), default=None)
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("report: no CUDA device -- libbonsai has no CPU fallback")
     parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "scaling": scaling,
-             "merger": merger, "mac": mac_variants}
+             "merger": merger, "mac": mac_variants, "issue_mix": issue_mix}
     doc = {k: f(args.reps) for k, f in parts.items() if args.only in (None, k)}
     print(json.dumps(doc, indent=1))
 
