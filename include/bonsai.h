@@ -125,7 +125,9 @@ int bonsai_walk(bonsai_ctx* ctx, float theta, float eps, const uint8_t* active_m
  * the first time a combination (pos_mass_dev, n, theta, eps, active_mask_dev, acc_pot_dev_out) is seen -- on a stream
  * the library owns, so the caller's stream may be the legacy default stream -- and replayed with one graph launch
  * from then on (the four most recent combinations are kept): below ~10^5 particles a step is bound by launch gaps
- * (P:L32).  The replay enqueues exactly the kernels of the staged calls; results are bit-identical.
+ * (P:L32).  The replay enqueues exactly the kernels of the staged calls; results are bit-identical.  The graph reads
+ * the buffers, not a snapshot of them: new particle data in the same buffers needs no new capture.  A caller that
+ * passes different buffers on every call gains nothing (16 misses in a row switch capturing off for the context).
  * EINVAL / ESTATE / ECUDA as the staged calls. */
 int bonsai_step(bonsai_ctx* ctx, const float* pos_mass_dev, uint32_t n, float theta, float eps,
                 const uint8_t* active_mask_dev, float* acc_pot_dev_out);

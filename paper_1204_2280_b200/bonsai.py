@@ -266,8 +266,12 @@ class Bonsai:
         assert pos_mass.dim() == 2 and pos_mass.shape[1] == 4
         n = pos_mass.shape[0]
         if out is None:
-            with torch.cuda.stream(self.stream):
-                out = torch.zeros((n, 4), dtype=torch.float32, device=self.device)
+            # a fresh result tensor per call would make every call a new graph (the buffers are part of the key):
+            # without a caller-owned `out` the step is enqueued kernel by kernel
+            self.load(pos_mass)
+            self.build_tree()
+            self.compute_multipoles()
+            return self.walk(theta, eps, active_mask, None)
         assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.shape == (n, 4)
         mptr = None
         if active_mask is not None:

@@ -199,6 +199,7 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.tree_auto = false;
     c.capture_stream = nullptr;
     c.graph_clock = c.graph_replays = 0;
+    c.graph_misses = 0;
     for (int k = 0; k < kGraphSlots; ++k) c.graphs[k].valid = false;
     // kernel attributes and occupancy are per device: set for every context (idempotent), never behind a
     // process-wide flag
@@ -350,9 +351,16 @@ int run_sequence(bonsai_ctx* h, const GraphKey& key, F&& enqueue) {
             restore_host_state(c, g.after);
             c->launches += g.launches;
             c->graph_replays += 1;
+            c->graph_misses = 0;
             g.last_use = c->graph_clock;
             return BONSAI_OK;
         }
+    }
+    // a caller that passes fresh buffers every call would pay a capture + instantiation each time: after 16 misses in
+    // a row the context stops capturing
+    if (++c->graph_misses > 16) {
+        c->prm.no_graph = 1;
+        return enqueue();
     }
     if (!c->capture_stream && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
         (void)cudaGetLastError();

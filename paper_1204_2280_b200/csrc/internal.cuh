@@ -199,6 +199,7 @@ struct Ctx {
     cudaStream_t capture_stream;  // library-owned stream the sequences are captured on (any caller stream can replay)
     GraphSlot graphs[kGraphSlots];
     uint64_t graph_clock, graph_replays;
+    uint32_t graph_misses;     // consecutive calls that found no captured graph (16 in a row switch capturing off)
     Gate gate;                 // applied to every launch of the build chain (bbox .. tree) while it is set (R30)
     bool tree_auto;            // the tree on the device was rebuilt OR refreshed by a device-side decision (R30)
     int walk_blocks_per_sm[8]; // occupancy of the k_walk instances on this device (set in bonsai_create)
