@@ -665,6 +665,7 @@ int bonsai_get_groups(bonsai_ctx* h, bonsai_groups_view* out) {
     if (!h || !out) return BONSAI_EINVAL;
     if (h->c.state < 2) return BONSAI_ESTATE;
     const Buffers& b = h->c.b;
+    if (h->c.groups_all_active) BONSAI_TRY(groups_fill_identity(&h->c));  // not materialised by the step itself
     out->n_groups = &b.ctl->n_groups;
     out->n_active = &b.ctl->n_active;
     out->active_list = b.active_list;

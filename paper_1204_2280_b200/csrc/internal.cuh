@@ -215,6 +215,7 @@ cudaError_t stage_reorder(Ctx* c, bool write_keys);
 cudaError_t stage_sort_ties(Ctx* c);
 cudaError_t stage_build(Ctx* c);
 cudaError_t stage_groups(Ctx* c, const uint8_t* mask_load_order);
+cudaError_t groups_fill_identity(Ctx* c);  // active_list of an all-active group list, on demand (introspection)
 cudaError_t stage_multipoles(Ctx* c);
 cudaError_t cells_qraw(Ctx* c);  // fills c_qraw from c_mom (introspection)
 cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out);

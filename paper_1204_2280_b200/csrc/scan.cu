@@ -1,6 +1,7 @@
 // Device-wide exclusive prefix sum of u32 (one of the "primitive algorithms" of P:L44 / P:L48 that the
-// sort, tree-build and group stages are assembled from).  Three launches: per-block sums, one block
-// scanning the block sums, per-block rescan with the carried-in offset.
+// sort, tree-build and group stages are assembled from).  Two launches: per-block sums, then a per-block rescan in
+// which every block first adds up the sums of the blocks before it (at most n / 2048 values, 8 KB at N = 2^22, out of
+// L2) -- cheaper than a third launch with a single block scanning the sums (round 1: 10 us + a launch gap).
 #include "internal.cuh"
 
 namespace bonsai {
@@ -46,20 +47,6 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_sums(const uint32_t* __re
     if (threadIdx.x == 0) sums[blockIdx.x] = total;
 }
 
-// single block: sums[0..m) -> exclusive, sums[m] = grand total
-__global__ void __launch_bounds__(kScanThreads) k_scan_top(uint32_t* __restrict__ sums, uint32_t m) {
-    uint32_t carry = 0;
-    for (uint32_t t0 = 0; t0 < m; t0 += kScanThreads) {
-        uint32_t t = t0 + threadIdx.x;
-        uint32_t v = (t < m) ? sums[t] : 0u;
-        uint32_t total;
-        uint32_t e = block_exclusive_scan(v, &total);
-        if (t < m) sums[t] = carry + e;
-        carry += total;
-    }
-    if (threadIdx.x == 0) sums[m] = carry;
-}
-
 __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* in, uint32_t* out, uint32_t n,
                                                              const uint32_t* __restrict__ sums, uint32_t m) {
     const uint32_t base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
@@ -70,22 +57,26 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* in,
         v[k] = (base + k < n) ? in[base + k] : 0u;
         s += v[k];
     }
+    // offset of this block = sum of the block sums before it (every block computes its own: no third kernel)
+    uint32_t before = 0;
+    for (uint32_t j = threadIdx.x; j < blockIdx.x; j += kScanThreads) before += sums[j];
+    uint32_t offset;
+    block_exclusive_scan(before, &offset);
     uint32_t total;
-    uint32_t run = block_exclusive_scan(s, &total) + sums[blockIdx.x];
+    uint32_t run = block_exclusive_scan(s, &total) + offset;
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k) {
         if (base + k < n) out[base + k] = run;
         run += v[k];
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = sums[m];
+    if (blockIdx.x == m - 1 && threadIdx.x == 0) out[n] = offset + total;  // the last block knows the grand total
 }
 
 cudaError_t exclusive_scan_u32(Ctx* c, const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* tmp) {
     const uint32_t m = div_up(n, kScanTile);
     k_scan_sums<<<m, kScanThreads, 0, c->stream>>>(in, n, tmp);
-    k_scan_top<<<1, kScanThreads, 0, c->stream>>>(tmp, m);
     k_scan_apply<<<m, kScanThreads, 0, c->stream>>>(in, out, n, tmp, m);
-    c->launches += 3;
+    c->launches += 2;
     return cudaGetLastError();
 }
 

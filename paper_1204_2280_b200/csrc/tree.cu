@@ -16,7 +16,7 @@
 //   lcp[e] < L <= leaf_level[e-1].  Breadth-first numbering = level offset + rank of the start among the
 //   level-L starts, so ids come from one per-level count/scan over blocks and warp ballots inside a block.
 //
-// Launches: k_tree_lcp, k_tree_levels (leaf levels + per-block per-level start counts),
+// Launches: k_tree_levels (lcp + leaf levels + per-block per-level start counts),
 // k_tree_scan_levels (prefix over blocks per level, level offsets, n_cells), k_tree_emit (cell records),
 // k_tree_finalize (count = end - first, n_child = last_child - first_child + 1).
 #include "internal.cuh"
@@ -34,19 +34,6 @@ __device__ __forceinline__ int common_digits(uint32_t ahi, uint32_t amid, uint32
     return 30;
 }
 
-__global__ void __launch_bounds__(256) k_tree_lcp(const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
-                                                  const uint32_t* __restrict__ klo, uint32_t n,
-                                                  int8_t* __restrict__ lcp, const Gate gate) {
-    if (gate_closed(gate)) return;
-    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i > n) return;
-    int v = -1;
-    if (i > 0 && i < n)
-        v = common_digits(__ldg(&khi[i - 1]), __ldg(&kmid[i - 1]), __ldg(&klo[i - 1]), __ldg(&khi[i]), __ldg(&kmid[i]),
-                          __ldg(&klo[i]));
-    lcp[i] = (int8_t)v;
-}
-
 // bits (lo_excl, hi_incl] of a 31-bit level mask; lo_excl may be -1
 __device__ __forceinline__ uint32_t level_range_mask(int lo_excl, int hi_incl) {
     if (hi_incl <= lo_excl) return 0u;
@@ -60,8 +47,14 @@ __device__ __forceinline__ uint32_t tree_item(uint32_t block, int w, int r, int 
     return block * kTreeTile + w * (32 * kTreeItems) + r * 32 + l;
 }
 
-__global__ void __launch_bounds__(kTreeThreads) k_tree_levels(const int8_t* __restrict__ lcp, uint32_t n, int nleaf,
-                                                              uint32_t n_blocks, int8_t* __restrict__ leaf_level,
+// lcp[] is computed here, from the sorted keys, for the block's span plus a halo of kMaxNleaf boundaries on each
+// side (the keys are read once more per halo -- 12 % more than a separate lcp pass, which this saves), and stored for
+// k_tree_emit.
+__global__ void __launch_bounds__(kTreeThreads) k_tree_levels(const uint32_t* __restrict__ khi,
+                                                              const uint32_t* __restrict__ kmid,
+                                                              const uint32_t* __restrict__ klo, uint32_t n, int nleaf,
+                                                              uint32_t n_blocks, int8_t* __restrict__ lcp,
+                                                              int8_t* __restrict__ leaf_level,
                                                               uint32_t* __restrict__ blk_level_count, const Gate gate) {
     constexpr int H = kMaxNleaf;
     if (gate_closed(gate)) return;
@@ -69,8 +62,13 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_levels(const int8_t* __re
     __shared__ uint32_t s_cnt[kLevelSlots];
     const long long base = (long long)blockIdx.x * kTreeTile;
     for (int j = threadIdx.x; j < kTreeTile + 2 * H + 1; j += kTreeThreads) {
-        long long b = base - H + j;
-        s_lcp[j] = (b >= 0 && b <= (long long)n) ? lcp[b] : (int8_t)-1;
+        const long long b = base - H + j;
+        int v = -1;  // boundaries 0 and n, and everything outside [0, n]
+        if (b > 0 && b < (long long)n)
+            v = common_digits(__ldg(&khi[b - 1]), __ldg(&kmid[b - 1]), __ldg(&klo[b - 1]), __ldg(&khi[b]), __ldg(&kmid[b]),
+                              __ldg(&klo[b]));
+        s_lcp[j] = (int8_t)v;
+        if (j >= H && j < H + kTreeTile && b <= (long long)n) lcp[b] = (int8_t)v;  // this block's own boundaries
     }
     if (threadIdx.x < kLevelSlots) s_cnt[threadIdx.x] = 0;
     __syncthreads();
@@ -105,18 +103,21 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_levels(const int8_t* __re
 
 // One block per level: exclusive prefix over blocks in place; the last block to finish turns the level totals
 // into level offsets and n_cells.
-__global__ void __launch_bounds__(256) k_tree_scan_levels(uint32_t* __restrict__ blk_level_count, uint32_t n_blocks,
-                                                          uint32_t* __restrict__ level_total, Control* __restrict__ ctl,
-                                                          uint32_t cap_cells, const Gate gate) {
-    __shared__ uint32_t wsum[8];
-    if (gate_closed(gate)) return;
+constexpr int kScanLvThreads = 1024;
+
+__global__ void __launch_bounds__(kScanLvThreads) k_tree_scan_levels(uint32_t* __restrict__ blk_level_count, uint32_t n_blocks,
+                                                                     uint32_t* __restrict__ level_total,
+                                                                     Control* __restrict__ ctl, uint32_t cap_cells,
+                                                                     const Gate gate) {
+    __shared__ uint32_t wsum[kScanLvThreads / 32];
     __shared__ uint32_t carry;
     __shared__ bool s_last;
+    if (gate_closed(gate)) return;
     uint32_t* row = blk_level_count + (size_t)blockIdx.x * n_blocks;
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
     const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (uint32_t t0 = 0; t0 < n_blocks; t0 += 256) {
+    for (uint32_t t0 = 0; t0 < n_blocks; t0 += kScanLvThreads) {
         const uint32_t t = t0 + threadIdx.x;
         const uint32_t v = (t < n_blocks) ? row[t] : 0u;
         uint32_t x = v;
@@ -127,11 +128,21 @@ __global__ void __launch_bounds__(256) k_tree_scan_levels(uint32_t* __restrict__
         }
         if (l == 31) wsum[w] = x;
         __syncthreads();
-        uint32_t pre = carry;
-        for (int k = 0; k < w; ++k) pre += wsum[k];
+        if (w == 0) {  // exclusive scan of the 32 warp totals
+            const uint32_t tw = wsum[l];
+            uint32_t y = tw;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t z = __shfl_up_sync(0xFFFFFFFFu, y, o);
+                if (l >= o) y += z;
+            }
+            wsum[l] = y - tw;
+        }
+        __syncthreads();
+        const uint32_t pre = carry + wsum[w];
         if (t < n_blocks) row[t] = pre + x - v;
         __syncthreads();
-        if (threadIdx.x == 255) carry = pre + x;
+        if (threadIdx.x == kScanLvThreads - 1) carry = pre + x;
         __syncthreads();
     }
     if (threadIdx.x == 0) {
@@ -266,15 +277,14 @@ cudaError_t stage_build(Ctx* c) {
     const int s = c->sorted_buf;
     const uint32_t n_blocks = div_up(n + 1, kTreeTile);
     CellArrays ca{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
-    k_tree_lcp<<<div_up(n + 1, 256), 256, 0, c->stream>>>(b.key[s][0], b.key[s][1], b.key[s][2], n, b.lcp, c->gate);
-    k_tree_levels<<<n_blocks, kTreeThreads, 0, c->stream>>>(b.lcp, n, (int)c->prm.nleaf, n_blocks, b.leaf_level,
-                                                            b.blk_level_count, c->gate);
-    k_tree_scan_levels<<<kMaxLevel + 1, 256, 0, c->stream>>>(b.blk_level_count, n_blocks, b.level_total, b.ctl,
+    k_tree_levels<<<n_blocks, kTreeThreads, 0, c->stream>>>(b.key[s][0], b.key[s][1], b.key[s][2], n, (int)c->prm.nleaf, n_blocks,
+                                                            b.lcp, b.leaf_level, b.blk_level_count, c->gate);
+    k_tree_scan_levels<<<kMaxLevel + 1, kScanLvThreads, 0, c->stream>>>(b.blk_level_count, n_blocks, b.level_total, b.ctl,
                                                              c->cap_cells, c->gate);
     k_tree_emit<<<n_blocks, kTreeThreads, 0, c->stream>>>(b.lcp, b.leaf_level, n, n_blocks, b.blk_level_count, b.ctl,
                                                           c->cap_cells, ca, c->gate);
     k_tree_finalize<<<min(div_up(c->cap_cells, 256), (uint32_t)c->num_sms * 16u), 256, 0, c->stream>>>(b.ctl, c->cap_cells, ca, c->gate);
-    c->launches += 5;
+    c->launches += 4;
     return cudaGetLastError();
 }
 

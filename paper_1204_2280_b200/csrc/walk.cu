@@ -282,7 +282,8 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
 #pragma unroll
     for (int k = 0; k < NS; ++k) {
         const uint32_t off = lane + 32u * k;
-        sidx[k] = __ldg(&a.active_list[sink_first + (off < ns ? off : 0u)]);
+        const uint32_t at = sink_first + (off < ns ? off : 0u);
+        sidx[k] = a.active_list ? __ldg(&a.active_list[at]) : at;  // nullptr: all particles active, identity
         const float4 p = __ldg(&a.pos[sidx[k]]);
         s.x[k] = p.x; s.y[k] = p.y; s.z[k] = p.z;
         smass[k] = p.w;
@@ -576,7 +577,7 @@ cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
     a.quad = b.c_quad;
     a.pos = b.sorted_pos;
     a.perm = c->perm;
-    a.active_list = b.active_list;
+    a.active_list = c->groups_all_active ? nullptr : b.active_list;
     a.g_first = b.g_first;
     a.g_count = b.g_count;
     a.g_bmin = b.g_bmin;
