@@ -27,7 +27,22 @@ __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, ui
     __shared__ bool s_last;
     if (gate_closed(gate)) return;
     float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    // four independent 16-byte loads in flight per thread: with one, the pass is latency-bound (13 % issue-active, 48
+    // long-scoreboard stalls per issue, 2.6 TB/s; profiles/r2_nonwalk_ncu.md)
+    const uint32_t stride = gridDim.x * blockDim.x;
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3u * stride < n; i += 4u * stride) {
+        float4 p[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) p[k] = __ldg(&pos[i + k * stride]);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            mn[0] = fminf(mn[0], p[k].x); mx[0] = fmaxf(mx[0], p[k].x);
+            mn[1] = fminf(mn[1], p[k].y); mx[1] = fmaxf(mx[1], p[k].y);
+            mn[2] = fminf(mn[2], p[k].z); mx[2] = fmaxf(mx[2], p[k].z);
+        }
+    }
+    for (; i < n; i += stride) {
         float4 p = __ldg(&pos[i]);
         mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
         mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
