@@ -14,10 +14,14 @@
 //   rejected internal  -> its child run is pushed.
 // Few groups (a small active subset): one group's walk is a serial chain of ~0.4 ms, so when there are fewer
 // groups than resident warps the kernel would last as long as its slowest group.  The warps of a block then form
-// TEAMS of S = 2, 4 or 8 (chosen on the device from the number of groups): every warp of a team runs the same
-// traversal of the same group (same opening tests, same lists, same counts) but evaluates only every S-th batch of
-// 32 interactions, and the team's partial sums are folded in a fixed order at the end.  The traversal is ~15 % of a
-// group's time, so a team of 8 finishes a group ~4x sooner.
+// TEAMS of S = 2, 4 or 8 (chosen on the device from the number of groups) that walk ONE group together: the stack of
+// sibling runs is shared by the team (the members' private stacks, concatenated); per round every member takes its
+// own four runs off the top (eight lanes per run, no scan), tests those cells, keeps the cells it accepts and the
+// leaves it opens in its OWN rings and evaluates them itself, and pushes the children of the cells it opens back
+// onto the shared stack (two team barriers per round: counts, then stack).  Traversal and evaluation are both
+// divided by S; the union of the members' lists is exactly the group's list, so counts are unchanged, and the
+// members' partial sums and counts are folded in member order at the end.  (Round 1 let every member repeat the
+// whole traversal and only divided the evaluation: the traversal, ~15 % of a group-walk, bounded a team of 8 at ~4x.)
 // Interaction kernels run in fp32 (FFMA + MUFU.RSQ); each batch of <= 32 sources is summed in fp32 starting
 // from zero and the batch total is added to an fp64 running total, which keeps the round-off of the long sum
 // out of the result at the cost of 4 DADD per 32 interactions.
@@ -35,6 +39,7 @@ struct WalkArgs {
     const uint32_t *g_first, *g_count;
     const float *g_bmin, *g_bmax;
     float inv_theta, eps2;
+    uint32_t warps_small, warps_big;  // resident warps of the 8-warp and of the 16-warp team kernel (regime choice)
     float4* out;             // load order
     uint32_t *n_pp, *n_pc;   // load order
 };
@@ -50,6 +55,7 @@ struct __align__(16) WarpSmem {
 };
 
 size_t walk_smem_bytes(uint32_t) { return sizeof(WarpSmem) * kWalkWarps; }
+constexpr int kWalkWarpsBig = 16;  // the team kernel for very few groups: one block of 16 warps per SM, teams of up to 16
 
 __device__ __forceinline__ float rsqrt_fast(float x) {
     float y;
@@ -267,15 +273,20 @@ __device__ __forceinline__ void team_barrier(int team, int warps) {
 
 // kTeam: this warp is member `slot` of a team of `tsize` warps (WarpSmem of member j = (&S)[j - slot]) that walks
 // the chunk together; see the header.  kTeam = false compiles to the single-warp walk.
+constexpr int kTeamRuns = 4;  // runs a team member takes per round: 4 x 8 lanes
 // kMono: R29 -- accepted cells act as monopoles only: (COM, M) is a point source like any particle, so it joins the
 // p-p ring and the p-c kernel is never called; lists and counts are those of the quadrupole walk.
 template <int NS, bool kZeroEps, bool kTeam, bool kMono>
 __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int lane, uint32_t sink_first, uint32_t ns,
                                            const float (&bmin)[3], const float (&bmax)[3], int team, int slot,
                                            int tsize) {
-    const uint32_t tmask = kTeam ? (uint32_t)(tsize - 1) : 0u;
-    const uint32_t uslot = (uint32_t)slot;
+    constexpr uint32_t tmask = 0u, uslot = 0u;  // (every warp evaluates all the batches of its own rings)
     const uint32_t lt = (1u << lane) - 1u;
+    // team scratch in member 0's shared memory (its sink_xyz area, free once the sinks are in registers):
+    // T[0] = entries on the shared stack, T[1 + j] = runs member j pushes this round
+    volatile uint32_t* T = reinterpret_cast<volatile uint32_t*>(&(&S)[-slot].sink_xyz[0][0]);
+    auto team_stack = [&](uint32_t e) -> uint32_t& { return (&S)[(int)(e / kWalkStack) - slot].stack[e % kWalkStack]; };
+    const uint32_t team_cap = (uint32_t)tsize * kWalkStack;
     Sinks<NS> s;
     uint32_t sidx[NS];
     float smass[NS];
@@ -306,9 +317,33 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
     uint32_t pc_r = 0, pc_w = 0, pp_r = 0, pp_w = 0;
     uint32_t npc = 0, npp = 0;
     int sp = 1;
-    if (lane == 0) S.stack[0] = 0u;  // the root alone: first = 0, n = 1
+    if (!kTeam || slot == 0) {
+        if (lane == 0) {
+            S.stack[0] = 0u;  // the root alone: first = 0, n = 1
+            if (kTeam) T[0] = 1u;
+        }
+    }
     bool ok = true;
     while (sp > 0) {
+        bool valid;
+        uint32_t cell;
+        int take = 0;
+        if constexpr (kTeam) {
+            team_barrier(team, tsize);  // (A) the stack and its size as the last round left them
+            sp = (int)T[0];
+            if (sp == 0) break;
+            // ---- pop: member `slot` takes runs slot * 4 .. slot * 4 + 3 from the top, eight lanes per run ----
+            take = min(sp, kTeamRuns * tsize);
+            const int r = slot * kTeamRuns + (lane >> 3);
+            uint32_t e = 0;
+            int cnt = 0;
+            if (r < take) {
+                e = team_stack((uint32_t)(sp - 1 - r));
+                cnt = (int)(e & 7u) + 1;
+            }
+            valid = (lane & 7) < cnt;
+            cell = (e >> 3) + (uint32_t)(lane & 7);
+        } else {
         __syncwarp();
         // ---- pop as many runs as fit into 32 lanes ----
         const int navail = min(sp, 32);
@@ -324,16 +359,17 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
             const int y = __shfl_up_sync(0xFFFFFFFFu, incl, o);
             if (lane >= o) incl += y;
         }
-        const bool take = (lane < navail) && (incl <= 32);
-        const int k_taken = __popc(__ballot_sync(0xFFFFFFFFu, take));
+        const bool take_run = (lane < navail) && (incl <= 32);
+        const int k_taken = __popc(__ballot_sync(0xFFFFFFFFu, take_run));
         const int total = __shfl_sync(0xFFFFFFFFu, incl, k_taken - 1);
         sp -= k_taken;
-        const uint32_t startbits = __reduce_or_sync(0xFFFFFFFFu, take ? (1u << (incl - cnt)) : 0u);
+        const uint32_t startbits = __reduce_or_sync(0xFFFFFFFFu, take_run ? (1u << (incl - cnt)) : 0u);
         const int j = __popc(startbits & (0xFFFFFFFFu >> (31 - lane))) - 1;
         const uint32_t ej = __shfl_sync(0xFFFFFFFFu, e, j);
         const int exj = __shfl_sync(0xFFFFFFFFu, incl - cnt, j);
-        const bool valid = lane < total;
-        const uint32_t cell = (ej >> 3) + (uint32_t)(lane - exj);
+        valid = lane < total;
+        cell = (ej >> 3) + (uint32_t)(lane - exj);
+        }
         // ---- opening test (R9), every operation rounded once, in this order ----
         bool accept = false, leaf = false;
         uint32_t link_first = 0, info = 0;
@@ -356,12 +392,28 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
         // ---- rejected internal cells: push their child runs ----
         const bool open = valid && !accept && !leaf;
         const uint32_t om = __ballot_sync(0xFFFFFFFFu, open);
+        if constexpr (kTeam) {
+            if (lane == 0) T[1 + slot] = (uint32_t)__popc(om);
+            team_barrier(team, tsize);  // (B) every member has read its runs and published its count
+            uint32_t off = 0, total = 0;
+            for (int j = 0; j < tsize; ++j) {
+                const uint32_t v = T[1 + j];
+                if (j < slot) off += v;
+                total += v;
+            }
+            const uint32_t base = (uint32_t)(sp - take);
+            if (base + total > team_cap) { ok = false; break; }  // the same decision in every member
+            if (open) team_stack(base + off + (uint32_t)__popc(om & lt)) = (link_first << 3) | (info - 1u);
+            if (slot == 0 && lane == 0) T[0] = base + total;
+            sp = (int)(base + total);
+        } else {
         if (open) {
             const int pos = sp + __popc(om & lt);
             if (pos < kWalkStack) S.stack[pos] = (link_first << 3) | (info - 1u);
         }
         sp += __popc(om);
         if (sp > kWalkStack) { ok = false; break; }
+        }
         // ---- accepted cells ----
         const bool acc = valid && accept;
         const uint32_t am = __ballot_sync(0xFFFFFFFFu, acc);
@@ -450,6 +502,10 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
                 park[(4 * k + 2) * 32 + lane] = s.az[k];
                 park[(4 * k + 3) * 32 + lane] = s.ph[k];
             }
+            if (lane == 0) {  // this member's share of the lists
+                S.leaf_first[0] = npc;
+                S.leaf_first[1] = npp;
+            }
         }
         team_barrier(team, tsize);  // every member's partials are parked
         if (slot == 0)
@@ -462,6 +518,8 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
                 s.az[k] += park[(4 * k + 2) * 32 + lane];
                 s.ph[k] += park[(4 * k + 3) * 32 + lane];
             }
+            npc += (&S)[j].leaf_first[0];
+            npp += (&S)[j].leaf_first[1];
         }
         team_barrier(team, tsize);  // ... and consumed: the rings are free for the next chunk
         if (slot != 0) return true;
@@ -520,28 +578,40 @@ __device__ __forceinline__ void walk_groups(WarpSmem& S, const WalkArgs& a, uint
     }
 }
 
+// Cost model of a team configuration: with dynamic tickets a walk lasts about ceil(n_groups S / warps) rounds of one
+// group-walk each, and a team of S shortens a group-walk to ~(0.05 + 0.95 / S) of a single warp's.  Returns the
+// cheapest S <= max_team (the smaller one on near-ties) and its cost.
+__device__ __forceinline__ int best_team(uint32_t n_groups, uint32_t warps, int max_team, float* cost_out) {
+    int tsize = 1;
+    float best = 3.0e38f;
+    for (int ts = 1; ts <= max_team; ts *= 2) {
+        const float rounds = (float)(((unsigned long long)n_groups * ts + warps - 1) / warps);
+        const float cost = rounds * (0.05f + 0.95f / (float)ts);
+        if (cost < 0.95f * best) { best = cost; tsize = ts; }
+    }
+    *cost_out = best;
+    return tsize;
+}
+
 // kTeams = false: the plain one-warp-per-group kernel (all particles active: always enough groups).
-// kTeams = true: launched for masked walks; picks the team size from the number of groups on the device.
-template <bool kZeroEps, bool kTeams, bool kMono>
-__global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
+// kTeams = true: launched for masked walks and small systems; picks the team size from the number of groups on the
+// device.  Two instances are launched back to back, blocks of 8 warps (3 per SM) and blocks of 16 warps (1 per SM,
+// teams of up to 16); both evaluate the same cost model on the same group count, the cheaper one does the walk, the
+// other returns at once.
+template <bool kZeroEps, bool kTeams, bool kMono, int kWarps>
+__global__ void __launch_bounds__(kWarps * 32, kWarps == kWalkWarps ? 3 : 1) k_walk(WalkArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ uint32_t s_team_g[kWalkWarps];
+    __shared__ uint32_t s_team_g[kWarps];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[w];
     const uint32_t n_groups = a.ctl->n_groups;
     if constexpr (kTeams) {
-        // team size S in {1, 2, 4, 8}: with dynamic tickets the kernel lasts about ceil(n_groups S / warps) rounds of
-        // one group-walk each, and a team of S shortens a group-walk to ~(0.15 + 0.85 / S) of a single warp's (the
-        // traversal, ~15 %, is repeated by every member; measured, profiles/r1f_configs.md).  Take the cheapest S,
-        // the smaller one on near-ties.
-        const uint32_t warps = gridDim.x * kWalkWarps;
-        int tsize = 1;
-        float best = 3.0e38f;
-        for (int ts = 1; ts <= kWalkWarps; ts *= 2) {
-            const float rounds = (float)(((unsigned long long)n_groups * ts + warps - 1) / warps);
-            const float cost = rounds * (0.15f + 0.85f / (float)ts);
-            if (cost < 0.95f * best) { best = cost; tsize = ts; }
-        }
+        float cost_small, cost_big;
+        const int t_small = best_team(n_groups, a.warps_small, kWalkWarps, &cost_small);
+        const int t_big = best_team(n_groups, a.warps_big, kWalkWarpsBig, &cost_big);
+        const bool big_wins = cost_big < 0.9f * cost_small;
+        if (big_wins != (kWarps == kWalkWarpsBig)) return;
+        const int tsize = big_wins ? t_big : t_small;
         if (tsize > 1) {
             walk_groups<kZeroEps, true, kMono>(S, a, n_groups, lane, w, tsize, s_team_g);
             return;
@@ -552,9 +622,13 @@ __global__ void __launch_bounds__(kWalkWarps * 32, 3) k_walk(WalkArgs a) {
 
 using WalkKernel = void (*)(WalkArgs);
 // index = (eps == 0) + 2 (team-capable) + 4 (monopole only)
-static const WalkKernel kWalkKernels[8] = {k_walk<false, false, false>, k_walk<true, false, false>, k_walk<false, true, false>,
-                                           k_walk<true, true, false>,   k_walk<false, false, true>, k_walk<true, false, true>,
-                                           k_walk<false, true, true>,   k_walk<true, true, true>};
+static const WalkKernel kWalkKernels[8] = {k_walk<false, false, false, kWalkWarps>, k_walk<true, false, false, kWalkWarps>,
+                                           k_walk<false, true, false, kWalkWarps>,  k_walk<true, true, false, kWalkWarps>,
+                                           k_walk<false, false, true, kWalkWarps>,  k_walk<true, false, true, kWalkWarps>,
+                                           k_walk<false, true, true, kWalkWarps>,   k_walk<true, true, true, kWalkWarps>};
+// the 16-warp team kernels: index = (eps == 0) + 2 (monopole only)
+static const WalkKernel kWalkKernelsBig[4] = {k_walk<false, true, false, kWalkWarpsBig>, k_walk<true, true, false, kWalkWarpsBig>,
+                                              k_walk<false, true, true, kWalkWarpsBig>,  k_walk<true, true, true, kWalkWarpsBig>};
 
 // Kernel attributes are per device (and cheap to set again): done for every context at creation, so a second
 // device or a second host thread in the same process never launches without the dynamic shared memory opt-in.
@@ -566,6 +640,9 @@ cudaError_t walk_prepare(Ctx* c) {
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->walk_blocks_per_sm[k], kWalkKernels[k], kWalkWarps * 32, smem)) != cudaSuccess) return e;
         if (c->walk_blocks_per_sm[k] < 1) c->walk_blocks_per_sm[k] = 1;
     }
+    for (int k = 0; k < 4; ++k)
+        if ((e = cudaFuncSetAttribute(kWalkKernelsBig[k], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)(sizeof(WarpSmem) * kWalkWarpsBig))) != cudaSuccess) return e;
     return cudaSuccess;
 }
 
@@ -598,8 +675,15 @@ cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
     const bool few_groups = !c->groups_all_active || 2ull * (c->n / c->prm.ncrit) <= resident_warps;
     const int which = ((a.eps2 == 0.0f) ? 1 : 0) + (few_groups ? 2 : 0) + (c->prm.order == 1 ? 4 : 0);
     const int grid = c->num_sms * c->walk_blocks_per_sm[which];
+    a.warps_small = (uint32_t)grid * kWalkWarps;
+    a.warps_big = (uint32_t)c->num_sms * kWalkWarpsBig;
     kWalkKernels[which]<<<grid, kWalkWarps * 32, smem, c->stream>>>(a);
     c->launches += 1;
+    if (few_groups) {  // the 16-warp instance: does the walk instead when teams of 16 pay (see k_walk)
+        const int big = ((a.eps2 == 0.0f) ? 1 : 0) + (c->prm.order == 1 ? 2 : 0);
+        kWalkKernelsBig[big]<<<c->num_sms, kWalkWarpsBig * 32, sizeof(WarpSmem) * kWalkWarpsBig, c->stream>>>(a);
+        c->launches += 1;
+    }
     return cudaGetLastError();
 }
 
