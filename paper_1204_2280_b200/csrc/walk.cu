@@ -65,7 +65,7 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
 
 // Packed fp32x2 arithmetic (sm_100: FFMA2 / FMUL2 / FADD2).  One instruction does the same IEEE operation on the
 // two halves of a 64-bit register pair, so a lane that holds two sinks spends ONE issue slot per operation for
-// both of them.  Measured on B200 (profiles/r1b_fp32_peak_microbench.txt): FFMA2 runs at half the instruction rate
+// both of them.  Measured on B200 (profiles/r2_microbench.md): FFMA2 runs at half the instruction rate
 // of FFMA -- the same 74 TFLOP/s -- which turns the interaction loops from issue-bound into FP32-pipe-bound.
 typedef unsigned long long f32x2;  // two fp32 values in one 64-bit register pair: .x = low half, .y = high half
 __device__ __forceinline__ f32x2 pack2(float lo, float hi) {
@@ -303,7 +303,7 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
     if constexpr (NS == 2) {
         // The packed loops want (-x0, -x1) etc. in ALIGNED register pairs.  Left as halves of the two float4 loads
         // above, ptxas re-pairs them with two MOVs per coordinate in every loop iteration (ALU-pipe slots that
-        // FFMA2 cannot overlap, profiles/r1c); a round trip through shared memory as 64-bit words makes each pair
+        // FFMA2 cannot overlap, profiles/r2_microbench.md); a round trip through shared memory as 64-bit words makes each pair
         // the destination of one LDS.64.
         S.sink_xyz[0][lane] = make_float2(-s.x[0], -s.x[1]);
         S.sink_xyz[1][lane] = make_float2(-s.y[0], -s.y[1]);
