@@ -517,6 +517,30 @@ def test_full_size_4m_sampled():
     print("4m sampled", r)
 
 
+def test_beyond_the_baseline_sizes_16m_sampled():
+    """Four times the largest BASELINE size (N = 2^24: 2048 sort tiles, working set 4x the L2, 0.5 GB of particles):
+    every structural stage bit-exact in full, multipoles <= 1 ulp, the walk on every 64th group."""
+    n, theta, eps = 1 << 24, 0.75, 0.0008
+    pm = W.plummer(n)
+    ref = O.build(pm)
+    b = Bonsai(n)
+    out = b.step(_dev(pm), theta, eps, None, _nan_out(n)).cpu().numpy()
+    b.sync()
+    check_structure(b, ref)
+    check_groups(b, ref)
+    check_walk_sampled(b, out, ref, theta, eps, stride=64, tag="beyond BASELINE: plummer 2^24")
+
+
+def test_empty_and_oversized_inputs_are_rejected():
+    b = Bonsai(100)
+    pm = _dev(W.plummer(100))
+    assert b._L.bonsai_load(b._h, pm.data_ptr(), 0) == -1          # n = 0
+    assert b._L.bonsai_load(b._h, pm.data_ptr(), 101) == -1        # n > n_max
+    assert b._L.bonsai_load(b._h, pm.data_ptr() + 4, 10) == -1     # misaligned
+    assert b._L.bonsai_step(b._h, pm.data_ptr(), 0, 0.75, 0.01, None, pm.data_ptr()) == -1
+    assert b._L.bonsai_step(b._h, None, 10, 0.75, 0.01, None, pm.data_ptr()) == -1
+
+
 @pytest.mark.parametrize("theta", [0.3, 0.5, 0.75, 1.0])
 def test_full_size_config1_256k_theta_sweep(theta):
     """BASELINE.json configs[1]: N = 2^18, eps 0.005, the whole theta sweep, against the oracle's walk (every 4th
