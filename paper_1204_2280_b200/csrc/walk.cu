@@ -669,10 +669,12 @@ cudaError_t stage_walk(Ctx* c, float theta, float eps, float4* acc_pot_out) {
     // reset the ticket and the interaction totals (adjacent fields of the control block)
     if ((e = cudaMemsetAsync(&b.ctl->walk_ticket, 0, sizeof(uint32_t), c->stream)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(&b.ctl->sum_pp, 0, 2 * sizeof(unsigned long long), c->stream)) != cudaSuccess) return e;
-    // a masked walk, or a small system, may have far fewer groups than resident warps: the team-capable kernel
-    // adapts on the device; n / ncrit is a lower bound of the all-active group count known on the host
+    // a masked walk, or a small system, may have fewer groups than resident warps: the team-capable kernel adapts on
+    // the device; n / ncrit is a lower bound of the all-active group count known on the host (measured at
+    // N = 2^17 / 2^18 / 2^19: teams 0.41 / 0.75 / 1.26 ms against 0.55 / 0.72 / 1.27 ms for the plain kernel, so the
+    // team kernel is taken up to one group per resident warp)
     const unsigned long long resident_warps = (unsigned long long)c->num_sms * c->walk_blocks_per_sm[2] * kWalkWarps;
-    const bool few_groups = !c->groups_all_active || 2ull * (c->n / c->prm.ncrit) <= resident_warps;
+    const bool few_groups = !c->groups_all_active || c->n / c->prm.ncrit <= resident_warps;
     const int which = ((a.eps2 == 0.0f) ? 1 : 0) + (few_groups ? 2 : 0) + (c->prm.order == 1 ? 4 : 0);
     const int grid = c->num_sms * c->walk_blocks_per_sm[which];
     a.warps_small = (uint32_t)grid * kWalkWarps;

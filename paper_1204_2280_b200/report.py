@@ -118,8 +118,9 @@ def block_step(reps: int) -> dict:
 
 def scaling(reps: int) -> dict:
     rows = {}
-    for name in ("plummer_32k", "plummer_256k", "plummer_1m", "plummer_4m"):
-        cfg = W.CONFIGS[name]
+    beyond = {"plummer_16m": dict(n=1 << 24, eps=0.0008, theta=0.75)}  # four times the paper's largest N (working set 4x L2)
+    for name in ("plummer_32k", "plummer_256k", "plummer_1m", "plummer_4m", "plummer_16m"):
+        cfg = W.CONFIGS.get(name) or beyond[name]
         n, eps, theta = cfg["n"], cfg["eps"], cfg["theta"]
         pm = torch.from_numpy(W.plummer(n)).cuda()
         b = Bonsai(n)
