@@ -126,12 +126,13 @@ def run_reference(args):
         return 0
     W, n, theta, eps = _workload(args.workload)
     pm = W.plummer(n)
-    # each step: the full pre-walk stages + a walk sample bounded to ~8 s
+    # each step: the full pre-walk stages (~1.5 s) + a walk sample bounded to ~4 s, so that the default 20 steps end
+    # within two minutes
     for _ in range(min(args.warmup, 1)):
         oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 2.0)
     ests, what = [], ""
     for _ in range(args.steps):
-        est, what = oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 8.0)
+        est, what = oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 4.0)
         ests.append(est)
     est = float(np.mean(ests))
     value = n / est

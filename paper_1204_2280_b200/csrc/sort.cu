@@ -166,10 +166,15 @@ __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict_
         for (int p = 0; p < kSortPasses; ++p) {  // pass p sorts digit p % 3 of word 1 + p / 3 (mid, then hi)
             const uint32_t d = (w[1 + p / 3] >> (kRadixBits * (p % 3))) & (kRadix - 1);
             // a warp whose 32 keys share the digit (the leading digits of clustered or pre-sorted input)
-            // adds once instead of serialising 32 same-address atomics
-            const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, d, 0);
-            if (__all_sync(0xFFFFFFFFu, valid && d == d0)) {
-                if (lane == 0) atomicAdd(&h[p * kRadix + d], 32u);
+            // adds once instead of serialising 32 same-address atomics; only the hi word's digits (levels 1-10) are
+            // ever that uniform, the mid word's are as good as random and skip the vote
+            if (p >= 3) {
+                const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, d, 0);
+                if (__all_sync(0xFFFFFFFFu, valid && d == d0)) {
+                    if (lane == 0) atomicAdd(&h[p * kRadix + d], 32u);
+                } else if (valid) {
+                    atomicAdd(&h[p * kRadix + d], 1u);
+                }
             } else if (valid) {
                 atomicAdd(&h[p * kRadix + d], 1u);
             }
