@@ -444,6 +444,25 @@ def test_graph_replay_is_bit_identical_to_the_staged_calls():
     assert b.stage_ms()["walk"] > 0
 
 
+def test_team_walks_are_deterministic():
+    """Team walks (several warps per group over a shared stack, partial sums folded in member order) give bit-identical
+    results and counts from run to run, for the 8-warp and the 16-warp team kernel."""
+    n = 1 << 17
+    pm = W.plummer(n)
+    d_pm = _dev(pm)
+    for n_active in (n // 16, n // 1024):                  # ~130 groups (teams of 8 / 16) and ~3 groups (teams of 16)
+        mask = _dev(W.active_mask(pm, n_active, "clustered"))
+        b = Bonsai(n)
+        out = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+        ref = b.step(d_pm, 0.75, 0.005, mask, out).clone()
+        cnt = b.counts()
+        for _ in range(5):
+            got = b.step(d_pm, 0.75, 0.005, mask, out)
+            assert torch.equal(got, ref)
+            c2 = b.counts()
+            assert np.array_equal(cnt[0], c2[0]) and np.array_equal(cnt[1], c2[1])
+
+
 def test_status_is_cleared_by_the_next_build():
     """A capacity overflow is reported by the bonsai_sync of that step and must not poison the context: the next
     bonsai_build_tree clears the sticky status and repairs the arrival counters the overflow left behind."""
