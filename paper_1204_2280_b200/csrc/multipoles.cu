@@ -120,6 +120,9 @@ __global__ void __launch_bounds__(128, 8) k_multipoles(const Control* __restrict
     // decided on the device (R30): the gate is open (or absent) when it was
     const bool grow = !gate_closed(grow_gate);
     uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    // a cell-capacity overflow leaves child links that point past the arrays: nothing downstream of the build may
+    // follow them (bonsai_sync reports the status; the next build recovers)
+    if (ctl->status != 0) return;
     if (c >= min(ctl->n_cells, cap_cells)) return;
     if (t.n_child[c] != 0) return;  // internal cells are produced by their last child
     {

@@ -605,6 +605,12 @@ __global__ void __launch_bounds__(kWarps * 32, kWarps == kWalkWarps ? 3 : 1) k_w
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     WarpSmem& S = reinterpret_cast<WarpSmem*>(smem_raw)[w];
     const uint32_t n_groups = a.ctl->n_groups;
+    // after a cell-capacity overflow in the build the child links of the tree point past the arrays: do not follow them
+    // (one read per block: the walk itself may raise the status later, and a team must not split over it)
+    __shared__ int s_status;
+    if (threadIdx.x == 0) s_status = a.ctl->status;
+    __syncthreads();
+    if (s_status != 0) return;
     if constexpr (kTeams) {
         float cost_small, cost_big;
         const int t_small = best_team(n_groups, a.warps_small, kWalkWarps, &cost_small);
