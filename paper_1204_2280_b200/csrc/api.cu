@@ -198,6 +198,8 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.gate = Gate{nullptr, 0u};
     c.tree_auto = false;
     c.capture_stream = nullptr;
+    c.side_stream = nullptr;
+    c.ev_fork = c.ev_join = nullptr;
     c.graph_clock = c.graph_replays = 0;
     c.graph_misses = 0;
     for (int k = 0; k < kGraphSlots; ++k) c.graphs[k].valid = false;
@@ -258,6 +260,47 @@ int bonsai_build_tree(bonsai_ctx* h) {
     c->tree_refreshed = false;
     c->tree_auto = false;
     c->state = 2;
+    return BONSAI_OK;
+}
+
+// bonsai_build_tree + bonsai_compute_multipoles as bonsai_step enqueues them: the group kernels (a4') and the
+// multipole pass (a5) both need only the finished tree and neither reads what the other writes, and both are
+// latency-bound, so the groups run on a side stream beside the multipole pass (fork / join by events; inside a
+// capture this becomes two branches of the graph).  The same kernels with the same arguments as the two calls, so
+// the results are bit-identical.  With stage timing on the two run one after the other, as the separate calls do.
+static int build_tree_and_multipoles(Ctx* c) {
+    if (c->state < 1) return BONSAI_ESTATE;
+    BONSAI_TRY(stage_recover(c));
+    int rc;
+    if ((rc = build_chain(c)) != BONSAI_OK) return rc;
+    bool fork = !c->timing;
+    if (fork && !c->side_stream) {
+        if (cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            (void)cudaGetLastError();
+            fork = false;
+        }
+    }
+    if (fork) {
+        cudaStream_t main_stream = c->stream;
+        BONSAI_TRY(cudaEventRecord(c->ev_fork, main_stream));
+        BONSAI_TRY(cudaStreamWaitEvent(c->side_stream, c->ev_fork, 0));
+        c->stream = c->side_stream;
+        const cudaError_t e = stage_groups(c, nullptr);
+        c->stream = main_stream;
+        BONSAI_TRY(e);
+        BONSAI_TRY(cudaEventRecord(c->ev_join, c->side_stream));
+        BONSAI_TRY(stage_multipoles(c));
+        BONSAI_TRY(cudaStreamWaitEvent(main_stream, c->ev_join, 0));
+    } else {
+        { StageTimer t(c, 5); BONSAI_TRY(stage_groups(c, nullptr)); }
+        { StageTimer t(c, 6); BONSAI_TRY(stage_multipoles(c)); }
+    }
+    c->tree_n = c->n;
+    c->tree_refreshed = false;
+    c->tree_auto = false;
+    c->state = 3;
     return BONSAI_OK;
 }
 
@@ -417,8 +460,7 @@ int bonsai_step(bonsai_ctx* h, const float* pos_mass_dev, uint32_t n, float thet
     return run_sequence(h, key, [&]() -> int {
         int rc;
         if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
-        if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
-        if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
+        if ((rc = build_tree_and_multipoles(&h->c)) != BONSAI_OK) return rc;
         return bonsai_walk(h, theta, eps, active_mask_dev, acc_pot_dev_out);
     });
 }
@@ -504,8 +546,7 @@ int bonsai_leapfrog_step(bonsai_ctx* h, float* pos_mass_dev, float* vel_dev, flo
         }
         int rc;
         if ((rc = bonsai_load(h, pos_mass_dev, n)) != BONSAI_OK) return rc;
-        if ((rc = bonsai_build_tree(h)) != BONSAI_OK) return rc;
-        if ((rc = bonsai_compute_multipoles(h)) != BONSAI_OK) return rc;
+        if ((rc = build_tree_and_multipoles(c)) != BONSAI_OK) return rc;
         if ((rc = bonsai_walk(h, theta, eps, nullptr, acc_pot_dev)) != BONSAI_OK) return rc;
         {
             StageTimer t(c, 8);
@@ -592,6 +633,9 @@ void bonsai_destroy(bonsai_ctx* h) {
     for (int k = 0; k < kGraphSlots; ++k)
         if (h->c.graphs[k].valid) cudaGraphExecDestroy(h->c.graphs[k].exec);
     if (h->c.capture_stream) cudaStreamDestroy(h->c.capture_stream);
+    if (h->c.side_stream) cudaStreamDestroy(h->c.side_stream);
+    if (h->c.ev_fork) cudaEventDestroy(h->c.ev_fork);
+    if (h->c.ev_join) cudaEventDestroy(h->c.ev_join);
     for (int s = 0; s < BONSAI_N_STAGES; ++s)
         for (int i = 0; i < kStageIntervals; ++i)
             for (int k = 0; k < 2; ++k)

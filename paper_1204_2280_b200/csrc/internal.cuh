@@ -197,6 +197,8 @@ struct Ctx {
     int num_sms;
     int device;                // the CUDA device the context was created on
     cudaStream_t capture_stream;  // library-owned stream the sequences are captured on (any caller stream can replay)
+    cudaStream_t side_stream;     // library-owned: the group kernels of bonsai_step run here, beside the multipole pass
+    cudaEvent_t ev_fork, ev_join; // fork / join of that branch (no timing)
     GraphSlot graphs[kGraphSlots];
     uint64_t graph_clock, graph_replays;
     uint32_t graph_misses;     // consecutive calls that found no captured graph (16 in a row switch capturing off)
