@@ -140,59 +140,75 @@ __device__ __forceinline__ void eval_pp_packed(WarpSmem& S, uint32_t r0, int nb,
     __syncwarp();
 }
 
-template <int NS, bool kZeroEps>
-__device__ __forceinline__ void eval_pp(WarpSmem& S, uint32_t r0, int nb, float eps2, Sinks<NS>& s) {
-    if constexpr (NS == 2) {
-        eval_pp_packed<kZeroEps>(S, r0, nb, eps2, s);
-    } else {
-    float ax[NS], ay[NS], az[NS], ph[NS];
-#pragma unroll
-    for (int k = 0; k < NS; ++k) ax[k] = ay[k] = az[k] = ph[k] = 0.0f;
-    const float4* src = &S.pp[r0 & 63u];
+// NS = 1 (a group of <= 32 sinks: the short last run of a container): one sink per lane would leave half of every
+// packed operation empty, and scalar FFMA gives the shared-memory loads, MUFU and loop control no FFMA2 shadow to hide
+// in (measured with ncrit = 32: 1.4x the time per interaction).  Instead the lane's ONE sink rides in both halves
+// and the two halves take two DIFFERENT sources: the rings are kept in pair layout (pair p = sources 2p, 2p + 1 stored
+// as (x0, x1, y0, y1) (z0, z1, m0, m1)), so every operand is an aligned register pair straight out of an LDS.128.
+// An odd batch is padded with a massless source far away (contributes exactly 0).
+constexpr float kPadFar = 1.0e15f;
+
+__device__ __forceinline__ void pp_put_pairs(WarpSmem& S, uint32_t slot, const float4 v) {
+    float* f = reinterpret_cast<float*>(S.pp);
+    const uint32_t t = slot & 63u, base = (t >> 1) * 8u + (t & 1u);
+    f[base] = v.x; f[base + 2] = v.y; f[base + 4] = v.z; f[base + 6] = v.w;
+}
+
+template <bool kZeroEps>
+__device__ __forceinline__ void eval_pp_pairs(WarpSmem& S, uint32_t r0, int nb, float eps2, int lane, Sinks<1>& s) {
+    if (nb & 1) {  // (tails only: full batches hold 32 sources)
+        if (lane == 0) pp_put_pairs(S, r0 + (uint32_t)nb, make_float4(kPadFar, kPadFar, kPadFar, 0.0f));
+        __syncwarp();
+    }
+    const f32x2 nsx = s.nx2, nsy = s.ny2, nsz = s.nz2;
+    const f32x2 e2 = bc(eps2);
+    f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
+    const float4* src = &S.pp[r0 & 63u];  // batches start at ring slot 0 or 32: pair-aligned, no wrap
+    const int np = (nb + 1) >> 1;
 #pragma unroll 4
-    for (int j = 0; j < nb; ++j) {
-        const float4 q = src[j];
-#pragma unroll
-        for (int k = 0; k < NS; ++k) {
-            const float dx = q.x - s.x[k], dy = q.y - s.y[k], dz = q.z - s.z[k];
-            float rinv;
-            if (kZeroEps) {  // eps = 0: the self term (and only it, R11) has r = 0 and must drop out
-                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                rinv = (r2 > 0.0f) ? rsqrt_fast(r2) : 0.0f;
-            } else {         // eps > 0: the self term adds exactly m/eps to ph and 0 to a; removed at the end
-                rinv = rsqrt_fast(fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2))));
-            }
-            const float mr = q.w * rinv;
-            const float rinv2 = rinv * rinv;
-            const float mr3 = mr * rinv2;
-            ph[k] += mr;
-            ax[k] = fmaf(mr3, dx, ax[k]);
-            ay[k] = fmaf(mr3, dy, ay[k]);
-            az[k] = fmaf(mr3, dz, az[k]);
+    for (int p = 0; p < np; ++p) {
+        const float4 u = src[2 * p], v = src[2 * p + 1];
+        const f32x2 dx = fadd2(pack2(u.x, u.y), nsx), dy = fadd2(pack2(u.z, u.w), nsy), dz = fadd2(pack2(v.x, v.y), nsz);
+        f32x2 rinv;
+        if (kZeroEps) {  // eps = 0: the self term (and only it, R11) has r = 0 and must drop out
+            const f32x2 r2 = ffma2(dx, dx, ffma2(dy, dy, fmul2(dz, dz)));
+            rinv = pack2((lo2(r2) > 0.0f) ? rsqrt_fast(lo2(r2)) : 0.0f, (hi2(r2) > 0.0f) ? rsqrt_fast(hi2(r2)) : 0.0f);
+        } else {         // eps > 0: the self term adds exactly m/eps to ph and 0 to a; removed at the end
+            rinv = rsqrt2(ffma2(dx, dx, ffma2(dy, dy, ffma2(dz, dz, e2))));
         }
+        const f32x2 mr = fmul2(pack2(v.z, v.w), rinv);
+        const f32x2 rinv2 = fmul2(rinv, rinv);
+        const f32x2 mr3 = fmul2(mr, rinv2);
+        ph = fadd2(ph, mr);
+        ax = ffma2(mr3, dx, ax);
+        ay = ffma2(mr3, dy, ay);
+        az = ffma2(mr3, dz, az);
     }
-#pragma unroll
-    for (int k = 0; k < NS; ++k) {
-        s.ax[k] += (double)ax[k]; s.ay[k] += (double)ay[k]; s.az[k] += (double)az[k]; s.ph[k] += (double)ph[k];
-    }
+    s.ax[0] += (double)(lo2(ax) + hi2(ax)); s.ay[0] += (double)(lo2(ay) + hi2(ay));
+    s.az[0] += (double)(lo2(az) + hi2(az)); s.ph[0] += (double)(lo2(ph) + hi2(ph));
     __syncwarp();
-    }
+}
+
+template <int NS, bool kZeroEps>
+__device__ __forceinline__ void eval_pp(WarpSmem& S, uint32_t r0, int nb, float eps2, int lane, Sinks<NS>& s) {
+    if constexpr (NS == 2) eval_pp_packed<kZeroEps>(S, r0, nb, eps2, s);
+    else eval_pp_pairs<kZeroEps>(S, r0, nb, eps2, lane, s);
 }
 
 template <int NS>
 __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t r0, int nb, int lane, Sinks<NS>& s) {
-    if (lane < nb) {
-        const uint32_t c = S.pc_ids[(r0 + lane) & 63];
-        const float4* m = reinterpret_cast<const float4*>(a.mac + c);
-        const float4* q = reinterpret_cast<const float4*>(a.quad + c);
-        S.pc[lane][0] = __ldg(m);
-        S.pc[lane][1] = __ldg(q);
-        float4 q1 = __ldg(q + 1);
-        q1.z = q1.z * a.eps2;  // tr eps^2: the softening term of the quadrupole (see CellQuad), once per cell
-        S.pc[lane][2] = q1;
-    }
-    __syncwarp();
     if constexpr (NS == 2) {
+        if (lane < nb) {
+            const uint32_t c = S.pc_ids[(r0 + lane) & 63];
+            const float4* m = reinterpret_cast<const float4*>(a.mac + c);
+            const float4* q = reinterpret_cast<const float4*>(a.quad + c);
+            S.pc[lane][0] = __ldg(m);
+            S.pc[lane][1] = __ldg(q);
+            float4 q1 = __ldg(q + 1);
+            q1.z = q1.z * a.eps2;  // tr eps^2: the softening term of the quadrupole (see CellQuad), once per cell
+            S.pc[lane][2] = q1;
+        }
+        __syncwarp();
         const f32x2 nsx = s.nx2, nsy = s.ny2, nsz = s.nz2;
         const f32x2 e2 = bc(a.eps2);
         f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
@@ -223,38 +239,58 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
         s.ax[1] += (double)hi2(ax); s.ay[1] += (double)hi2(ay); s.az[1] += (double)hi2(az); s.ph[1] += (double)hi2(ph);
         __syncwarp();
     } else {
-    float ax[NS], ay[NS], az[NS], ph[NS];
-#pragma unroll
-    for (int k = 0; k < NS; ++k) ax[k] = ay[k] = az[k] = ph[k] = 0.0f;
-#pragma unroll 2
-    for (int j = 0; j < nb; ++j) {
-        const float4 c0 = S.pc[j][0], c1 = S.pc[j][1], c2 = S.pc[j][2];
-#pragma unroll
-        for (int k = 0; k < NS; ++k) {
-            const float dx = c0.x - s.x[k], dy = c0.y - s.y[k], dz = c0.z - s.z[k];
-            const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, a.eps2)));
-            const float rinv = rsqrt_fast(r2);
-            const float rinv2 = rinv * rinv;
-            const float prx = fmaf(c1.x, dx, fmaf(c1.w, dy, c2.x * dz));
-            const float pry = fmaf(c1.w, dx, fmaf(c1.y, dy, c2.y * dz));
-            const float prz = fmaf(c2.x, dx, fmaf(c2.y, dy, c1.z * dz));
-            const float sq = fmaf(dx, prx, fmaf(dy, pry, fmaf(dz, prz, c2.z)));
-            const float rinv3 = rinv * rinv2;
-            const float rinv5 = rinv3 * rinv2;
-            const float q5 = sq * rinv5;
-            ph[k] = fmaf(c0.w, rinv, ph[k]);
-            ph[k] = fmaf(-0.5f, q5, ph[k]);
-            const float f = fmaf(-2.5f, q5 * rinv2, c0.w * rinv3);
-            ax[k] = fmaf(dx, f, ax[k]); ax[k] = fmaf(rinv5, prx, ax[k]);
-            ay[k] = fmaf(dy, f, ay[k]); ay[k] = fmaf(rinv5, pry, ay[k]);
-            az[k] = fmaf(dz, f, az[k]); az[k] = fmaf(rinv5, prz, az[k]);
+        // pair layout (see eval_pp_pairs): pair p = cells 2p, 2p + 1 as six float4
+        //   (cx0, cx1, cy0, cy1) (cz0, cz1, M0, M1) (Pxx0, Pxx1, Pyy0, Pyy1) (Pzz0, Pzz1, Pxy0, Pxy1)
+        //   (Pxz0, Pxz1, Pyz0, Pyz1) (tr0 eps^2, tr1 eps^2, -, -);  S.pc holds 16 pairs
+        float* f = reinterpret_cast<float*>(S.pc);
+        if (lane < nb) {
+            const uint32_t c = S.pc_ids[(r0 + lane) & 63];
+            const float4* m = reinterpret_cast<const float4*>(a.mac + c);
+            const float4* q = reinterpret_cast<const float4*>(a.quad + c);
+            const float4 m0 = __ldg(m), q0 = __ldg(q), q1 = __ldg(q + 1);
+            const uint32_t base = ((uint32_t)lane >> 1) * 24u + ((uint32_t)lane & 1u);
+            f[base] = m0.x; f[base + 2] = m0.y; f[base + 4] = m0.z; f[base + 6] = m0.w;
+            f[base + 8] = q0.x; f[base + 10] = q0.y; f[base + 12] = q0.z; f[base + 14] = q0.w;
+            f[base + 16] = q1.x; f[base + 18] = q1.y; f[base + 20] = q1.z * a.eps2;
+        } else if (lane == nb && (nb & 1)) {  // odd tail: a massless cell far away contributes exactly 0
+            const uint32_t base = ((uint32_t)lane >> 1) * 24u + 1u;
+            f[base] = kPadFar; f[base + 2] = kPadFar; f[base + 4] = kPadFar; f[base + 6] = 0.0f;
+            f[base + 8] = 0.0f; f[base + 10] = 0.0f; f[base + 12] = 0.0f; f[base + 14] = 0.0f;
+            f[base + 16] = 0.0f; f[base + 18] = 0.0f; f[base + 20] = 0.0f;
         }
-    }
-#pragma unroll
-    for (int k = 0; k < NS; ++k) {
-        s.ax[k] += (double)ax[k]; s.ay[k] += (double)ay[k]; s.az[k] += (double)az[k]; s.ph[k] += (double)ph[k];
-    }
-    __syncwarp();
+        __syncwarp();
+        const f32x2 nsx = s.nx2, nsy = s.ny2, nsz = s.nz2;
+        const f32x2 e2 = bc(a.eps2);
+        f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
+        const float4* src = &S.pc[0][0];
+        const int np = (nb + 1) >> 1;
+#pragma unroll 2
+        for (int p = 0; p < np; ++p) {
+            const float4 A = src[6 * p], B = src[6 * p + 1], C = src[6 * p + 2], D = src[6 * p + 3], E = src[6 * p + 4],
+                         F = src[6 * p + 5];
+            const f32x2 dx = fadd2(pack2(A.x, A.y), nsx), dy = fadd2(pack2(A.z, A.w), nsy), dz = fadd2(pack2(B.x, B.y), nsz);
+            const f32x2 M = pack2(B.z, B.w);
+            const f32x2 pxx = pack2(C.x, C.y), pyy = pack2(C.z, C.w), pzz = pack2(D.x, D.y), pxy = pack2(D.z, D.w),
+                        pxz = pack2(E.x, E.y), pyz = pack2(E.z, E.w);
+            const f32x2 rinv = rsqrt2(ffma2(dx, dx, ffma2(dy, dy, ffma2(dz, dz, e2))));
+            const f32x2 rinv2 = fmul2(rinv, rinv);
+            const f32x2 prx = ffma2(pxx, dx, ffma2(pxy, dy, fmul2(pxz, dz)));
+            const f32x2 pry = ffma2(pxy, dx, ffma2(pyy, dy, fmul2(pyz, dz)));
+            const f32x2 prz = ffma2(pxz, dx, ffma2(pyz, dy, fmul2(pzz, dz)));
+            const f32x2 sq = ffma2(dx, prx, ffma2(dy, pry, ffma2(dz, prz, pack2(F.x, F.y))));  // dr.P.dr + tr eps^2
+            const f32x2 rinv3 = fmul2(rinv, rinv2);
+            const f32x2 rinv5 = fmul2(rinv3, rinv2);
+            const f32x2 q5 = fmul2(sq, rinv5);
+            ph = ffma2(M, rinv, ph);
+            ph = ffma2(bc(-0.5f), q5, ph);
+            const f32x2 g = ffma2(bc(-2.5f), fmul2(q5, rinv2), fmul2(M, rinv3));
+            ax = ffma2(dx, g, ax); ax = ffma2(rinv5, prx, ax);
+            ay = ffma2(dy, g, ay); ay = ffma2(rinv5, pry, ay);
+            az = ffma2(dz, g, az); az = ffma2(rinv5, prz, az);
+        }
+        s.ax[0] += (double)(lo2(ax) + hi2(ax)); s.ay[0] += (double)(lo2(ay) + hi2(ay));
+        s.az[0] += (double)(lo2(az) + hi2(az)); s.ph[0] += (double)(lo2(ph) + hi2(ph));
+        __syncwarp();
     }
 }
 
@@ -313,6 +349,11 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
         asm volatile("ld.shared.b64 %0, [%1];" : "=l"(s.nx2) : "r"(sa));
         asm volatile("ld.shared.b64 %0, [%1];" : "=l"(s.ny2) : "r"(sa + 256u));
         asm volatile("ld.shared.b64 %0, [%1];" : "=l"(s.nz2) : "r"(sa + 512u));
+    }
+    if constexpr (NS == 1) {  // the one sink in both halves (eval_pp_pairs)
+        s.nx2 = pack2(-s.x[0], -s.x[0]);
+        s.ny2 = pack2(-s.y[0], -s.y[0]);
+        s.nz2 = pack2(-s.z[0], -s.z[0]);
     }
     uint32_t pc_r = 0, pc_w = 0, pp_r = 0, pp_w = 0;
     uint32_t npc = 0, npp = 0;
@@ -421,13 +462,16 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
             if (am) {
                 if (acc) {
                     const uint32_t slot_w = pp_w + __popc(am & lt);
-                    if (!kTeam || ((slot_w >> 5) & tmask) == uslot) S.pp[slot_w & 63u] = m0;  // (COM, M)
+                    if (!kTeam || ((slot_w >> 5) & tmask) == uslot) {  // (COM, M)
+                        if constexpr (NS == 1) pp_put_pairs(S, slot_w, m0);
+                        else S.pp[slot_w & 63u] = m0;
+                    }
                 }
                 pp_w += __popc(am);
                 npc += __popc(am);
                 __syncwarp();
                 if (pp_w - pp_r >= 32u) {
-                    if (!kTeam || ((pp_r >> 5) & tmask) == uslot) eval_pp<NS, kZeroEps>(S, pp_r, 32, a.eps2, s);
+                    if (!kTeam || ((pp_r >> 5) & tmask) == uslot) eval_pp<NS, kZeroEps>(S, pp_r, 32, a.eps2, lane, s);
                     pp_r += 32u;
                 }
             }
@@ -471,13 +515,16 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
                 const int before = __popc(__ballot_sync(0xFFFFFFFFu, oleaf && lpre < base));
                 if (t < T) {
                     const int r = before + __popc(starts & (0xFFFFFFFFu >> (31 - lane))) - 1;
-                    if (!kTeam || (((pp_w + lane) >> 5) & tmask) == uslot)  // only the batches this member evaluates
-                        S.pp[(pp_w + lane) & 63u] = __ldg(&a.pos[S.leaf_first[r] + (t - S.leaf_pref[r])]);
+                    if (!kTeam || (((pp_w + lane) >> 5) & tmask) == uslot) {  // only the batches this member evaluates
+                        const float4 src = __ldg(&a.pos[S.leaf_first[r] + (t - S.leaf_pref[r])]);
+                        if constexpr (NS == 1) pp_put_pairs(S, pp_w + lane, src);
+                        else S.pp[(pp_w + lane) & 63u] = src;
+                    }
                 }
                 pp_w += min(32u, T - base);
                 __syncwarp();
                 if (pp_w - pp_r >= 32u) {
-                    if (!kTeam || ((pp_r >> 5) & tmask) == uslot) eval_pp<NS, kZeroEps>(S, pp_r, 32, a.eps2, s);
+                    if (!kTeam || ((pp_r >> 5) & tmask) == uslot) eval_pp<NS, kZeroEps>(S, pp_r, 32, a.eps2, lane, s);
                     pp_r += 32u;
                 }
             }
@@ -487,7 +534,7 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
     __syncwarp();
     if (pc_w != pc_r && (!kTeam || ((pc_r >> 5) & tmask) == uslot)) eval_pc<NS>(S, a, pc_r, (int)(pc_w - pc_r), lane, s);
     if (pp_w != pp_r && (!kTeam || ((pp_r >> 5) & tmask) == uslot))
-        eval_pp<NS, kZeroEps>(S, pp_r, (int)(pp_w - pp_r), a.eps2, s);
+        eval_pp<NS, kZeroEps>(S, pp_r, (int)(pp_w - pp_r), a.eps2, lane, s);
     if (kTeam) {
         // fold the members' partial sums: each member parks its 4 NS doubles per lane in its own source rings
         // (dead now), member 0 adds them in member order
