@@ -106,6 +106,7 @@ struct Sinks {
     f32x2 nx2, ny2, nz2;     // NS = 2: (-x0, -x1), (-y0, -y1), (-z0, -z1), kept packed for the whole walk
     float x[NS], y[NS], z[NS];
     double ax[NS], ay[NS], az[NS], ph[NS];  // ph accumulates +sum m/r (negated on output)
+    int pair0, pair_step;    // NS = 1: this lane evaluates the source pairs pair0, pair0 + pair_step, ... (lane split)
 };
 
 // NS = 2: the two sinks of a lane ride in the two halves of packed registers; operation for operation (and
@@ -165,8 +166,9 @@ __device__ __forceinline__ void eval_pp_pairs(WarpSmem& S, uint32_t r0, int nb, 
     f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
     const float4* src = &S.pp[r0 & 63u];  // batches start at ring slot 0 or 32: pair-aligned, no wrap
     const int np = (nb + 1) >> 1;
+    const int pstep = s.pair_step;
 #pragma unroll 4
-    for (int p = 0; p < np; ++p) {
+    for (int p = s.pair0; p < np; p += pstep) {
         const float4 u = src[2 * p], v = src[2 * p + 1];
         const f32x2 dx = fadd2(pack2(u.x, u.y), nsx), dy = fadd2(pack2(u.z, u.w), nsy), dz = fadd2(pack2(v.x, v.y), nsz);
         f32x2 rinv;
@@ -264,8 +266,9 @@ __device__ __forceinline__ void eval_pc(WarpSmem& S, const WalkArgs& a, uint32_t
         f32x2 ax = bc(0.0f), ay = bc(0.0f), az = bc(0.0f), ph = bc(0.0f);
         const float4* src = &S.pc[0][0];
         const int np = (nb + 1) >> 1;
+        const int pstep = s.pair_step;
 #pragma unroll 2
-        for (int p = 0; p < np; ++p) {
+        for (int p = s.pair0; p < np; p += pstep) {
             const float4 A = src[6 * p], B = src[6 * p + 1], C = src[6 * p + 2], D = src[6 * p + 3], E = src[6 * p + 4],
                          F = src[6 * p + 5];
             const f32x2 dx = fadd2(pack2(A.x, A.y), nsx), dy = fadd2(pack2(A.z, A.w), nsy), dz = fadd2(pack2(B.x, B.y), nsz);
@@ -326,9 +329,20 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
     Sinks<NS> s;
     uint32_t sidx[NS];
     float smass[NS];
+    // Lane split (NS = 1): a group of ns <= 16 sinks would leave half of the lanes (or more) idle.  With m = the
+    // smallest power of two >= ns, lane l holds sink l mod m and is replica l / m of 32 / m; replica r evaluates the
+    // source pairs r, r + 32/m, ... of every batch, and the replicas' partial sums are added by a butterfly at the end.
+    uint32_t split_m = 32u;
+    if constexpr (NS == 1) {
+        while (split_m > 1u && (split_m >> 1) >= ns) split_m >>= 1;
+        s.pair_step = (int)(32u / split_m);
+        s.pair0 = lane / (int)split_m;
+    }
 #pragma unroll
     for (int k = 0; k < NS; ++k) {
-        const uint32_t off = lane + 32u * k;
+        // NS = 1 with ns <= 16: the sinks are replicated over the lanes (sink = lane mod m, m = the power of two >= ns)
+        // and the 32 / m replicas share the sources of every batch between them -- see the lane split below
+        const uint32_t off = (NS == 1 ? ((uint32_t)lane & (split_m - 1u)) : (uint32_t)lane) + 32u * k;
         const uint32_t at = sink_first + (off < ns ? off : 0u);
         sidx[k] = a.active_list ? __ldg(&a.active_list[at]) : at;  // nullptr: all particles active, identity
         const float4 p = __ldg(&a.pos[sidx[k]]);
@@ -535,6 +549,14 @@ __device__ __forceinline__ bool walk_chunk(WarpSmem& S, const WalkArgs& a, int l
     if (pc_w != pc_r && (!kTeam || ((pc_r >> 5) & tmask) == uslot)) eval_pc<NS>(S, a, pc_r, (int)(pc_w - pc_r), lane, s);
     if (pp_w != pp_r && (!kTeam || ((pp_r >> 5) & tmask) == uslot))
         eval_pp<NS, kZeroEps>(S, pp_r, (int)(pp_w - pp_r), a.eps2, lane, s);
+    if constexpr (NS == 1) {  // lane split: add the replicas' partial sums (every replica ends with the same bits)
+        for (uint32_t o = split_m; o < 32u; o <<= 1) {
+            s.ax[0] += __shfl_xor_sync(0xFFFFFFFFu, s.ax[0], o);
+            s.ay[0] += __shfl_xor_sync(0xFFFFFFFFu, s.ay[0], o);
+            s.az[0] += __shfl_xor_sync(0xFFFFFFFFu, s.az[0], o);
+            s.ph[0] += __shfl_xor_sync(0xFFFFFFFFu, s.ph[0], o);
+        }
+    }
     if (kTeam) {
         // fold the members' partial sums: each member parks its 4 NS doubles per lane in its own source rings
         // (dead now), member 0 adds them in member order
