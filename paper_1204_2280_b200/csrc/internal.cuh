@@ -74,6 +74,8 @@ struct Control {
     uint32_t look_wrap;          // the epoch wrapped: k_sort_gscan clears the look-back table
     uint32_t long_ticket;        // run scheduler / last-warp-done counter of k_sort_long_runs
     uint32_t long_done;
+    uint32_t mult_ticket;        // tile scheduler of k_multipoles (tiles of cells, deepest first)
+    uint32_t mult_done;          // ... and its last-block-out counter, which resets both
 };
 
 // A launch that only does its work when a device flag has a given value.  The flag is written by an earlier kernel
