@@ -71,6 +71,9 @@ typedef struct {
     float rebuild_factor;/* [1.25] bonsai_block_tick(rebuild = -1) rebuilds the tree when the interactions per
                             walked sink of the last walk exceed rebuild_factor x those of the first walk after the
                             last build (R30); >= 1                                                       */
+    uint32_t mult_kernel;/* [0] which of the two multipole kernels runs (same results to the last bit of the fp64 sums'
+                            rounding order within a cell): 0 = by size (tiles from n = 2^21), 1 = the last child to
+                            arrive climbs (small systems), 2 = tiles of cells deepest first, parents wait            */
 } bonsai_params;
 
 /* Bytes of device workspace bonsai_create() needs for up to n_max particles (0 on bad arguments). */

@@ -5,12 +5,10 @@
 // centre| and the geometric side l.  Everything is accumulated in fp64 and rounded ONCE to fp32, because the
 // fp32 opening test of the walk must see the same COM / delta as the reference to the last bit (R9).
 //
-// One launch, bottom-up without level barriers: a thread per cell; leaves sum their particles (in particle order,
-// without FMA contraction), then every thread climbs: it bumps its parent's arrival counter and the LAST child
-// to arrive combines the children's fp64 moments (parallel-axis shift about the parent's COM; moments about
-// the origin would cancel catastrophically in the halo) and continues upward.  Nobody waits on anybody.
-// (A persistent grid with one grid barrier per level, eight lanes per internal cell, measured 0.30 ms against
-// 0.28 ms for this scheme at N = 2^22: the leaf phase is latency-bound either way, the barriers add load imbalance.)
+// One launch, bottom-up without level barriers: a lane per cell, tiles of 32 cells handed out deepest-first; leaves sum
+// their particles (in particle order, without FMA contraction), internal cells wait until their children have
+// published and combine the children's fp64 moments (parallel-axis shift about the parent's COM; moments about
+// the origin would cancel catastrophically in the halo).  See k_multipoles for the scheduling argument.
 // The exact fp32 bounding box of every cell's members rides along; a refreshed tree (R25) uses it to let l
 // grow when particles have drifted out of their cell.
 #include "internal.cuh"
@@ -107,16 +105,155 @@ struct TreeView {
     const uint32_t *level, *first, *count, *first_child, *n_child, *parent;
 };
 
-// Block scheduler: tiles of 128 consecutive cells are handed out by an atomic ticket from the END of the cell array
-// (breadth-first numbering: children have larger ids than their parent, so the deepest cells come first).  A block that
-// holds ticket t therefore knows that every tile with children of its cells has been STARTED by a running block, and
+// Leaf: sums over its particles, in particle order, without FMA contraction.
+template <bool kBox>
+__device__ __forceinline__ void leaf_moments(const float4* __restrict__ sorted_pos, uint32_t f, uint32_t cnt, Mom& q,
+                                             float (&mn)[3], float (&mx)[3]) {
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+    q.m = 0.0;
+    q.cx = q.cy = q.cz = 0.0;
+    q.xx = q.yy = q.zz = q.xy = q.xz = q.yz = 0.0;
+    for (uint32_t k = 0; k < cnt; ++k) {
+        const float4 p = __ldg(&sorted_pos[f + k]);
+        const double m = (double)p.w;
+        if (kBox) {
+            mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
+            mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
+            mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
+        }
+        q.m = __dadd_rn(q.m, m);
+        sx = __dadd_rn(sx, __dmul_rn(m, (double)p.x));
+        sy = __dadd_rn(sy, __dmul_rn(m, (double)p.y));
+        sz = __dadd_rn(sz, __dmul_rn(m, (double)p.z));
+    }
+    if (q.m > 0.0) {
+        q.cx = sx / q.m; q.cy = sy / q.m; q.cz = sz / q.m;
+        for (uint32_t k = 0; k < cnt; ++k) {
+            const float4 p = __ldg(&sorted_pos[f + k]);
+            const double m = (double)p.w;
+            const double dx = __dadd_rn((double)p.x, -q.cx), dy = __dadd_rn((double)p.y, -q.cy),
+                         dz = __dadd_rn((double)p.z, -q.cz);
+            q.xx = __dadd_rn(q.xx, __dmul_rn(__dmul_rn(m, dx), dx));
+            q.yy = __dadd_rn(q.yy, __dmul_rn(__dmul_rn(m, dy), dy));
+            q.zz = __dadd_rn(q.zz, __dmul_rn(__dmul_rn(m, dz), dz));
+            q.xy = __dadd_rn(q.xy, __dmul_rn(__dmul_rn(m, dx), dy));
+            q.xz = __dadd_rn(q.xz, __dmul_rn(__dmul_rn(m, dx), dz));
+            q.yz = __dadd_rn(q.yz, __dmul_rn(__dmul_rn(m, dy), dz));
+        }
+    }
+}
+
+// Internal cell: ONE pass over the children's fp64 records (each fetched once, two children's loads in flight per
+// trip).  Moments are gathered about the first child's centre c0 -- at most a cell diagonal away from every other child,
+// so the shift to the centre of mass below cancels at most one digit of the fp64 sums -- and moved to the COM at the
+// end (parallel-axis theorem):
+//   M = sum m_k,  S = sum m_k d_k,  T = sum (Q_k + m_k d_k d_k^T),  d_k = c_k - c0;
+//   COM = c0 + S / M,  Q = T - M (S / M)(S / M)^T.
+// A massless child has Q = 0 and m = 0 and drops out by itself.
+template <bool kBox>
+__device__ __forceinline__ void combine_children(const double* __restrict__ c_mom, const float* __restrict__ c_box, uint32_t fc,
+                                                 uint32_t nc, Mom& q, float (&mn)[3], float (&mx)[3]) {
+    const double2* mo0 = reinterpret_cast<const double2*>(c_mom + (size_t)fc * 10);
+    double c0x = 0.0, c0y = 0.0, c0z = 0.0;
+    double M = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
+    double txx = 0.0, tyy = 0.0, tzz = 0.0, txy = 0.0, txz = 0.0, tyz = 0.0;
+#pragma unroll 2
+    for (uint32_t k = 0; k < nc; ++k) {
+        const double2 r0 = __ldcg(&mo0[5 * k + 0]), r1 = __ldcg(&mo0[5 * k + 1]), r2 = __ldcg(&mo0[5 * k + 2]),
+                      r3 = __ldcg(&mo0[5 * k + 3]), r4 = __ldcg(&mo0[5 * k + 4]);
+        if (kBox) {
+            const float2* bx = reinterpret_cast<const float2*>(c_box + (size_t)(fc + k) * 6);
+            const float2 b0 = __ldcg(&bx[0]), b1 = __ldcg(&bx[1]), b2 = __ldcg(&bx[2]);
+            mn[0] = fminf(mn[0], b0.x); mn[1] = fminf(mn[1], b0.y); mn[2] = fminf(mn[2], b1.x);
+            mx[0] = fmaxf(mx[0], b1.y); mx[1] = fmaxf(mx[1], b2.x); mx[2] = fmaxf(mx[2], b2.y);
+        }
+        if (k == 0) { c0x = r0.y; c0y = r1.x; c0z = r1.y; }
+        const double m = r0.x;
+        const double dx = r0.y - c0x, dy = r1.x - c0y, dz = r1.y - c0z;
+        M += m;
+        sx += m * dx; sy += m * dy; sz += m * dz;
+        txx += r2.x + m * dx * dx;
+        tyy += r2.y + m * dy * dy;
+        tzz += r3.x + m * dz * dz;
+        txy += r3.y + m * dx * dy;
+        txz += r4.x + m * dx * dz;
+        tyz += r4.y + m * dy * dz;
+    }
+    q.m = M;
+    q.cx = q.cy = q.cz = 0.0;
+    q.xx = q.yy = q.zz = q.xy = q.xz = q.yz = 0.0;
+    if (M > 0.0) {
+        const double ux = sx / M, uy = sy / M, uz = sz / M;
+        q.cx = c0x + ux; q.cy = c0y + uy; q.cz = c0z + uz;
+        q.xx = txx - M * ux * ux;
+        q.yy = tyy - M * uy * uy;
+        q.zz = tzz - M * uz * uz;
+        q.xy = txy - M * ux * uy;
+        q.xz = txz - M * ux * uz;
+        q.yz = tyz - M * uy * uz;
+    }
+}
+
+// Small systems (n < kMultTilesMinN): one thread per cell, the LAST child to arrive at a parent combines its siblings
+// and climbs on -- nobody waits.  Most of the time one lane per warp is active, but the chain from the deepest leaf
+// to the root (which is all a small tree has) is one acq_rel atomic + one round of loads per level, shorter than the
+// publish / poll hand-off of the tiled kernel below: 0.056 against 0.078 ms at N = 2^15, 0.097 against 0.107 ms at 2^20.
+template <bool kBox, bool kTight>
+__global__ void __launch_bounds__(128, 8) k_multipoles_climb(Control* __restrict__ ctl, uint32_t cap_cells, TreeView t,
+                                                    const float4* __restrict__ sorted_pos,
+                                                    const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
+                                                    const uint32_t* __restrict__ klo, double* __restrict__ c_mom,
+                                                    CellMac* __restrict__ c_mac, CellQuad* __restrict__ c_quad,
+                                                    float* __restrict__ c_qraw, float* __restrict__ c_box,
+                                                    uint32_t* __restrict__ c_arrived, const Gate grow_gate) {
+    const bool grow = !gate_closed(grow_gate);  // (see k_multipoles)
+    uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ctl->status != 0) return;               // (see k_multipoles)
+    if (c >= min(ctl->n_cells, cap_cells)) return;
+    if (t.n_child[c] != 0) return;  // internal cells are produced by their last child
+    {
+        const uint32_t f = t.first[c], cnt = t.count[c];
+        Mom q;
+        float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+        leaf_moments<kBox>(sorted_pos, f, cnt, q, mn, mx);
+        store_cell<kBox, kTight>(q, mn, mx, c, (int)t.level[c], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, f,
+                   kLeafBit | cnt, c_mom, c_box, c_mac, c_quad, c_qraw, grow);
+    }
+    for (;;) {
+        const uint32_t p = t.parent[c];
+        if (p == kNone) return;
+        const uint32_t nc = t.n_child[p];
+        // release: this cell's moments are visible (gpu scope) before the arrival is; acquire: the last child to
+        // arrive sees its siblings' moments.  One acq_rel atomic instead of two full fences around a relaxed one.
+        uint32_t arrived;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(arrived) : "l"(&c_arrived[p]) : "memory");
+        if (arrived + 1u != nc) return;
+        c_arrived[p] = 0;  // ready for the next step
+        const uint32_t fc = t.first_child[p];
+        Mom q;
+        float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+        combine_children<kBox>(c_mom, c_box, fc, nc, q, mn, mx);
+        const uint32_t f = t.first[p];
+        store_cell<kBox, kTight>(q, mn, mx, p, (int)t.level[p], __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, fc, nc,
+                   c_mom, c_box, c_mac, c_quad, c_qraw, grow);
+        c = p;
+    }
+}
+
+// Scheduler: tiles of 32 consecutive cells, one per warp, are handed out by an atomic ticket from the END of the cell
+// array (breadth-first numbering: children have larger ids than their parent, so the deepest cells come first).  A warp
+// that holds ticket t therefore knows that every tile with children of its cells has been STARTED by a running warp, and
 // may wait for them: an internal cell spins (acquire) on its arrival counter until all children have published their
-// moments (release).  Waiting is rare -- the children's tiles were drawn thousands of tickets earlier -- except near the
-// root.  Inside a tile the levels are processed deepest first with a block barrier in between (a tile can hold a parent
-// and its children only near the root, where levels are shorter than a tile).
+// moments (release: one gpu-scope fence per warp after a warp barrier, then relaxed increments).  Waiting is rare -- the
+// children's tiles were drawn thousands of tickets earlier -- except near the root.  Inside a tile the levels are
+// processed deepest first with a warp barrier in between (a tile can hold a parent and its children only near the root,
+// where levels are shorter than a tile).  No block-wide barrier anywhere: the warps of a block are independent.
 // (Until round 2 the last child to arrive combined its siblings and climbed on: one active lane per warp for most of
-// the kernel, 28 % of the warp slots in use, 0.204 ms at N = 2^22.)
+// the kernel, 28 % of the warp slots in use, 0.204 ms at N = 2^22; tiles of 128 cells per block with block barriers:
+// 0.178 ms, 15 % of the stall samples at the barrier and 6 % in per-thread release fences; this form: 0.173 ms.
+// Fetching the leaf particles two or four at a time spills at 64 registers: 0.198 / 0.219 ms.)
 constexpr int kMultThreads = 128;
+constexpr uint32_t kMultTilesMinN = 1u << 21;  // below: k_multipoles_climb (measured crossover between 2^20 and 2^22)
 
 template <bool kBox, bool kTight>
 __global__ void __launch_bounds__(kMultThreads, 8) k_multipoles(Control* __restrict__ ctl, uint32_t cap_cells, TreeView t,
@@ -133,139 +270,60 @@ __global__ void __launch_bounds__(kMultThreads, 8) k_multipoles(Control* __restr
     // follow them (bonsai_sync reports the status; the next build recovers)
     if (ctl->status != 0) return;
     const uint32_t n_cells = min(ctl->n_cells, cap_cells);
-    const uint32_t n_tiles = (n_cells + kMultThreads - 1) / kMultThreads;
-    __shared__ uint32_t s_ticket;
-    __shared__ int s_lmax, s_lmin;
+    const uint32_t n_tiles = (n_cells + 31u) / 32u;
+    const int lane = threadIdx.x & 31;
     for (;;) {
-        __syncthreads();  // the previous tile is done with the shared variables
-        if (threadIdx.x == 0) {
-            s_ticket = atomicAdd(&ctl->mult_ticket, 1u);
-            s_lmax = -1;
-            s_lmin = 64;
-        }
-        __syncthreads();
-        const uint32_t ticket = s_ticket;
+        uint32_t ticket = 0;
+        if (lane == 0) ticket = atomicAdd(&ctl->mult_ticket, 1u);
+        ticket = __shfl_sync(0xFFFFFFFFu, ticket, 0);
         if (ticket >= n_tiles) break;
-        const uint32_t c = (n_tiles - 1u - ticket) * kMultThreads + threadIdx.x;
+        const uint32_t c = (n_tiles - 1u - ticket) * 32u + (uint32_t)lane;
         const bool valid = c < n_cells;
         const int level = valid ? (int)t.level[c] : -1;
-        if (valid) {
-            atomicMax(&s_lmax, level);
-            atomicMin(&s_lmin, level);
-        }
-        __syncthreads();
-        const int lmax = s_lmax, lmin = s_lmin;
+        const int lmax = __reduce_max_sync(0xFFFFFFFFu, level);
+        const int lmin = __reduce_min_sync(0xFFFFFFFFu, valid ? level : 64);
         for (int L = lmax; L >= lmin; --L) {
-            if (valid && level == L) {
+            const bool mine = valid && level == L;
+            uint32_t parent = kNone;
+            if (mine) {
                 const uint32_t nc = t.n_child[c];
                 Mom q;
                 float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
-                q.cx = q.cy = q.cz = 0.0;
-                q.xx = q.yy = q.zz = q.xy = q.xz = q.yz = 0.0;
                 const uint32_t f = t.first[c];
                 uint32_t link_first, link_info;
                 if (nc == 0) {
-                    // ---- leaf: sums over its particles, in particle order, without FMA contraction ----
                     const uint32_t cnt = t.count[c];
-                    double sx = 0.0, sy = 0.0, sz = 0.0;
-                    q.m = 0.0;
-                    for (uint32_t k = 0; k < cnt; ++k) {
-                        const float4 p = __ldg(&sorted_pos[f + k]);
-                        const double m = (double)p.w;
-                        if (kBox) {
-                            mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
-                            mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
-                            mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
-                        }
-                        q.m = __dadd_rn(q.m, m);
-                        sx = __dadd_rn(sx, __dmul_rn(m, (double)p.x));
-                        sy = __dadd_rn(sy, __dmul_rn(m, (double)p.y));
-                        sz = __dadd_rn(sz, __dmul_rn(m, (double)p.z));
-                    }
-                    if (q.m > 0.0) {
-                        q.cx = sx / q.m; q.cy = sy / q.m; q.cz = sz / q.m;
-                        for (uint32_t k = 0; k < cnt; ++k) {
-                            const float4 p = __ldg(&sorted_pos[f + k]);
-                            const double m = (double)p.w;
-                            const double dx = __dadd_rn((double)p.x, -q.cx), dy = __dadd_rn((double)p.y, -q.cy),
-                                         dz = __dadd_rn((double)p.z, -q.cz);
-                            q.xx = __dadd_rn(q.xx, __dmul_rn(__dmul_rn(m, dx), dx));
-                            q.yy = __dadd_rn(q.yy, __dmul_rn(__dmul_rn(m, dy), dy));
-                            q.zz = __dadd_rn(q.zz, __dmul_rn(__dmul_rn(m, dz), dz));
-                            q.xy = __dadd_rn(q.xy, __dmul_rn(__dmul_rn(m, dx), dy));
-                            q.xz = __dadd_rn(q.xz, __dmul_rn(__dmul_rn(m, dx), dz));
-                            q.yz = __dadd_rn(q.yz, __dmul_rn(__dmul_rn(m, dy), dz));
-                        }
-                    }
+                    leaf_moments<kBox>(sorted_pos, f, cnt, q, mn, mx);
                     link_first = f;
                     link_info = kLeafBit | cnt;
                 } else {
-                    // ---- internal cell: wait for the children (acquire), then combine their fp64 moments ----
+                    // internal cell: wait for the children (acquire), then combine their fp64 moments
                     uint32_t arrived;
                     for (;;) {
                         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(arrived) : "l"(&c_arrived[c]) : "memory");
                         if (arrived == nc) break;
-                        __nanosleep(200);
+                        __nanosleep(40);
                     }
                     c_arrived[c] = 0;  // ready for the next step
                     const uint32_t fc = t.first_child[c];
-                    // ONE pass over the children (each record fetched once, two children's loads in flight per trip).
-                    // Moments are gathered about the first child's centre c0 -- at most a cell diagonal away from every
-                    // other child, so the shift to the centre of mass below cancels at most one digit of the fp64 sums
-                    // -- and moved to the COM at the end (parallel-axis theorem):
-                    //   M = sum m_k,  S = sum m_k d_k,  T = sum (Q_k + m_k d_k d_k^T),  d_k = c_k - c0;
-                    //   COM = c0 + S / M,  Q = T - M (S / M)(S / M)^T.
-                    // A massless child has Q = 0 and m = 0 and drops out by itself.
-                    const double2* mo0 = reinterpret_cast<const double2*>(c_mom + (size_t)fc * 10);
-                    double c0x = 0.0, c0y = 0.0, c0z = 0.0;
-                    double M = 0.0, sx = 0.0, sy = 0.0, sz = 0.0;
-                    double txx = 0.0, tyy = 0.0, tzz = 0.0, txy = 0.0, txz = 0.0, tyz = 0.0;
-#pragma unroll 2
-                    for (uint32_t k = 0; k < nc; ++k) {
-                        const double2 r0 = __ldcg(&mo0[5 * k + 0]), r1 = __ldcg(&mo0[5 * k + 1]), r2 = __ldcg(&mo0[5 * k + 2]),
-                                      r3 = __ldcg(&mo0[5 * k + 3]), r4 = __ldcg(&mo0[5 * k + 4]);
-                        if (kBox) {
-                            const float2* bx = reinterpret_cast<const float2*>(c_box + (size_t)(fc + k) * 6);
-                            const float2 b0 = __ldcg(&bx[0]), b1 = __ldcg(&bx[1]), b2 = __ldcg(&bx[2]);
-                            mn[0] = fminf(mn[0], b0.x); mn[1] = fminf(mn[1], b0.y); mn[2] = fminf(mn[2], b1.x);
-                            mx[0] = fmaxf(mx[0], b1.y); mx[1] = fmaxf(mx[1], b2.x); mx[2] = fmaxf(mx[2], b2.y);
-                        }
-                        if (k == 0) { c0x = r0.y; c0y = r1.x; c0z = r1.y; }
-                        const double m = r0.x;
-                        const double dx = r0.y - c0x, dy = r1.x - c0y, dz = r1.y - c0z;
-                        M += m;
-                        sx += m * dx; sy += m * dy; sz += m * dz;
-                        txx += r2.x + m * dx * dx;
-                        tyy += r2.y + m * dy * dy;
-                        tzz += r3.x + m * dz * dz;
-                        txy += r3.y + m * dx * dy;
-                        txz += r4.x + m * dx * dz;
-                        tyz += r4.y + m * dy * dz;
-                    }
-                    q.m = M;
-                    if (M > 0.0) {
-                        const double ux = sx / M, uy = sy / M, uz = sz / M;
-                        q.cx = c0x + ux; q.cy = c0y + uy; q.cz = c0z + uz;
-                        q.xx = txx - M * ux * ux;
-                        q.yy = tyy - M * uy * uy;
-                        q.zz = tzz - M * uz * uz;
-                        q.xy = txy - M * ux * uy;
-                        q.xz = txz - M * ux * uz;
-                        q.yz = tyz - M * uy * uz;
-                    }
+                    combine_children<kBox>(c_mom, c_box, fc, nc, q, mn, mx);
                     link_first = fc;
                     link_info = nc;
                 }
                 store_cell<kBox, kTight>(q, mn, mx, c, L, __ldg(&khi[f]), __ldg(&kmid[f]), __ldg(&klo[f]), ctl, link_first,
                                          link_info, c_mom, c_box, c_mac, c_quad, c_qraw, grow);
-                // release: this cell's moments (and box) are visible at gpu scope before the arrival is
-                const uint32_t p = t.parent[c];
-                if (p != kNone) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&c_arrived[p]) : "memory");
+                parent = t.parent[c];
             }
-            if (L > lmin) __syncthreads();  // (block-uniform condition)
+            // release, once per warp: the warp barrier orders the lanes' stores before lane 0's gpu-scope fence
+            // (cumulative), the arrivals after it may then be relaxed
+            __syncwarp();
+            if (lane == 0) __threadfence();
+            __syncwarp();
+            if (parent != kNone) asm volatile("red.relaxed.gpu.global.add.u32 [%0], 1;" ::"l"(&c_arrived[parent]) : "memory");
         }
     }
     // the last block to leave resets the scheduler for the next pass
+    __syncthreads();
     if (threadIdx.x == 0 && atomicAdd(&ctl->mult_done, 1u) == gridDim.x - 1) {
         ctl->mult_done = 0;
         ctl->mult_ticket = 0;
@@ -313,17 +371,26 @@ cudaError_t stage_multipoles(Ctx* c) {
     Buffers& b = c->b;
     const int s = c->sorted_buf;
     TreeView t{b.c_level, b.c_first, b.c_count, b.c_first_child, b.c_n_child, b.c_parent};
-    // persistent blocks (8 per SM) draw tiles of 128 cells until the device-side cell count is exhausted
-    const dim3 grid(min(div_up(c->cap_cells, (uint32_t)kMultThreads), (uint32_t)c->num_sms * 8u));
     using Kernel = void (*)(Control*, uint32_t, TreeView, const float4*, const uint32_t*, const uint32_t*, const uint32_t*,
                             double*, CellMac*, CellQuad*, float*, float*, uint32_t*, Gate);
-    const Kernel k = (c->prm.mac_mode == 1)              ? (Kernel)k_multipoles<true, true>
-                     : (c->tree_refreshed || c->tree_auto) ? (Kernel)k_multipoles<true, false>
-                                                           : (Kernel)k_multipoles<false, false>;
+    const int which = (c->prm.mac_mode == 1) ? 2 : (c->tree_refreshed || c->tree_auto) ? 1 : 0;
+    static const Kernel kTiles[3] = {k_multipoles<false, false>, k_multipoles<true, false>, k_multipoles<true, true>};
+    static const Kernel kClimb[3] = {k_multipoles_climb<false, false>, k_multipoles_climb<true, false>,
+                                     k_multipoles_climb<true, true>};
     // a tree handled by the device-side rebuild decision (R30) was refreshed iff rebuild_flag == 0
     const Gate grow = c->tree_auto ? Gate{&b.ctl->rebuild_flag, 0u} : Gate{nullptr, 0u};
-    k<<<grid, kMultThreads, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1], b.key[s][2], b.c_mom,
-                                   b.c_mac, b.c_quad, b.c_qraw, b.c_box, b.c_arrived, grow);
+    const bool tiles = c->prm.mult_kernel == 2 || (c->prm.mult_kernel == 0 && c->n >= kMultTilesMinN);
+    if (tiles) {
+        // persistent blocks (8 per SM) draw tiles of 32 cells until the device-side cell count is exhausted
+        const dim3 grid(min(div_up(c->cap_cells, (uint32_t)kMultThreads), (uint32_t)c->num_sms * 8u));
+        kTiles[which]<<<grid, kMultThreads, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0], b.key[s][1],
+                                                            b.key[s][2], b.c_mom, b.c_mac, b.c_quad, b.c_qraw, b.c_box,
+                                                            b.c_arrived, grow);
+    } else {
+        kClimb[which]<<<div_up(c->cap_cells, 128u), 128, 0, c->stream>>>(b.ctl, c->cap_cells, t, b.sorted_pos, b.key[s][0],
+                                                                         b.key[s][1], b.key[s][2], b.c_mom, b.c_mac, b.c_quad,
+                                                                         b.c_qraw, b.c_box, b.c_arrived, grow);
+    }
     c->launches += 1;
     return cudaGetLastError();
 }
