@@ -423,13 +423,19 @@ def run_ours(args):
 
 
 # Algorithmic bytes per particle of the HBM-bound stages (SURVEY.md section 8(d) floors):
-#   keys: 16 in + 3 key words out; sort: 6 pair passes over the mid and hi words x (8 in + 8 out), minus the index
-#   read of the first pass (iota) and the key write of the last; reorder: perm + record in, record + 3 key words out,
+#   keys: 16 in + 3 key words out; sort: P pair passes (P = 4 up to n = 2^22, 5 up to 2^25, else 6: the library's rule,
+#   csrc/sort.cu sort_first_pass) x (8 in + 8 out), minus the index read of the first pass (iota) and the key write of
+#   the last; reorder: perm + record in, record + 3 key words out,
 #   plus the tie check re-reading the hi and mid words; build: the single-pass floor, 12 (keys once) + 4 (cell
 #   records, 0.23 cells x 16 B); groups: positions once + one box per group; multipoles: positions once + 0.23 cells
 #   x 48 B out + the children's records re-read by the internal cells (~0.05 x 48 B) = 30.
+def sort_passes(a):
+    n = _workload(a.workload)[1]
+    return 4 if n <= (1 << 22) else 5 if n <= (1 << 25) else 6
+
+
 ALG_BYTES = {
-    "bbox": lambda a: 16, "keys": lambda a: 28, "sort": lambda a: 6 * 16 - 8, "reorder": lambda a: 48 + 8,
+    "bbox": lambda a: 16, "keys": lambda a: 28, "sort": lambda a: sort_passes(a) * 16 - 8, "reorder": lambda a: 48 + 8,
     "build": lambda a: 16, "groups": lambda a: 16 + 24 / a.ncrit, "multipoles": lambda a: 30,
 }
 

@@ -74,6 +74,10 @@ typedef struct {
     uint32_t mult_kernel;/* [0] which of the two multipole kernels runs (same results to the last bit of the fp64 sums'
                             rounding order within a cell): 0 = by size (tiles from n = 2^21), 1 = the last child to
                             arrive climbs (small systems), 2 = tiles of cells deepest first, parents wait            */
+    uint32_t sort_passes;/* [0] radix passes of the key sort (a2): 4, 5 or 6 passes of 10 bits over the leading 40, 50 or 60
+                            key bits; particles that agree in those are put in order of their remaining bits after the
+                            reorder (the permutation is the same bit for bit).  0 = by size: 4 up to n = 2^22, 5 up to
+                            2^25, else 6 (a strongly clustered system wants more passes)                             */
 } bonsai_params;
 
 /* Bytes of device workspace bonsai_create() needs for up to n_max particles (0 on bad arguments). */

@@ -40,7 +40,7 @@ class Params(C.Structure):
     _fields_ = [("nleaf", C.c_uint32), ("ncrit", C.c_uint32), ("group_mode", C.c_uint32),
                 ("cap_cells", C.c_uint32), ("group_cell", C.c_uint32), ("mac_mode", C.c_uint32),
                 ("order", C.c_uint32), ("no_graph", C.c_uint32), ("rebuild_factor", C.c_float),
-                ("mult_kernel", C.c_uint32)]
+                ("mult_kernel", C.c_uint32), ("sort_passes", C.c_uint32)]
 
 
 class CellsView(C.Structure):
@@ -197,7 +197,7 @@ class Bonsai:
     def __init__(self, n_max: int, nleaf: int = 16, ncrit: int = 64, group_mode: int = 2,
                  cap_cells: int = 0, group_cell: int = 0, device: str | torch.device = "cuda:0",
                  stream: "torch.cuda.Stream | None" = None, mac_mode: int = 0, order: int = 2,
-                 rebuild_factor: float = 0.0, use_graph: bool = True, mult_kernel: int = 0):
+                 rebuild_factor: float = 0.0, use_graph: bool = True, mult_kernel: int = 0, sort_passes: int = 0):
         if not torch.cuda.is_available():
             raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
         self.device = torch.device(device)
@@ -205,7 +205,7 @@ class Bonsai:
         self.n_max = int(n_max)
         self.n = 0
         self.params = Params(nleaf, ncrit, group_mode, cap_cells, group_cell, mac_mode, order, 0 if use_graph else 1,
-                             rebuild_factor, mult_kernel)
+                             rebuild_factor, mult_kernel, sort_passes)
         nbytes = int(self._L.bonsai_workspace_bytes(self.n_max, C.byref(self.params)))
         if nbytes == 0:
             raise BonsaiError(EINVAL, "bonsai_workspace_bytes")

@@ -30,10 +30,11 @@ struct Carver {
 
 bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out) {
     bonsai_params p;
-    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0; p.mac_mode = 0; p.order = 2; p.rebuild_factor = 0.0f; p.no_graph = 0; p.mult_kernel = 0;
+    p.nleaf = 16; p.ncrit = 64; p.group_mode = 2; p.cap_cells = 0; p.group_cell = 0; p.mac_mode = 0; p.order = 2; p.rebuild_factor = 0.0f; p.no_graph = 0; p.mult_kernel = 0; p.sort_passes = 0;
     if (in) {
         p.no_graph = in->no_graph;
         p.mult_kernel = in->mult_kernel;
+        p.sort_passes = in->sort_passes;
         p.rebuild_factor = in->rebuild_factor;
         p.mac_mode = in->mac_mode;
         if (in->order) p.order = in->order;
@@ -55,6 +56,7 @@ bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out)
     if (p.ncrit < 1 || p.ncrit > (uint32_t)kMaxNcrit) return false;
     if (p.group_mode > 2) return false;
     if (p.mac_mode > 1 || p.order < 1 || p.order > 2 || p.mult_kernel > 2) return false;
+    if (p.sort_passes != 0 && (p.sort_passes < 4 || p.sort_passes > 6)) return false;
     if (p.rebuild_factor == 0.0f) p.rebuild_factor = 1.25f;
     if (!(p.rebuild_factor >= 1.0f) || std::isinf(p.rebuild_factor)) return false;
     if (p.cap_cells < 1 || p.cap_cells >= (1u << 29)) return false;  // walk stack entries pack the id into 29 bits

@@ -215,6 +215,7 @@ inline uint32_t div_up(uint32_t a, uint32_t b) { return (a + b - 1) / b; }
 cudaError_t stage_bbox(Ctx* c);
 cudaError_t stage_keys(Ctx* c);
 cudaError_t stage_sort(Ctx* c);
+int sort_first_pass(const Ctx* c);  // the passes sort_first_pass() .. 5 run (params.sort_passes, else a rule on n)
 cudaError_t stage_reorder(Ctx* c, bool write_keys);
 cudaError_t stage_sort_ties(Ctx* c);
 cudaError_t stage_build(Ctx* c);

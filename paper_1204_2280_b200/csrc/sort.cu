@@ -144,7 +144,7 @@ __device__ __forceinline__ void morton_words(const float4 p, const float lox, co
 __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict__ pos, uint32_t n,
                                                        const Control* __restrict__ ctl, uint32_t* __restrict__ khi,
                                                        uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
-                                                       uint32_t* __restrict__ ghist, const Gate gate) {
+                                                       uint32_t* __restrict__ ghist, const int first_pass, const Gate gate) {
     __shared__ uint32_t h[kSortPasses * kRadix];
     if (gate_closed(gate)) return;
     for (int k = threadIdx.x; k < kSortPasses * kRadix; k += kKeysThreads) h[k] = 0;
@@ -164,6 +164,7 @@ __global__ void __launch_bounds__(kKeysThreads) k_keys(const float4* __restrict_
         }
 #pragma unroll
         for (int p = 0; p < kSortPasses; ++p) {  // pass p sorts digit p % 3 of word 1 + p / 3 (mid, then hi)
+            if (p < first_pass) continue;        // (the lowest mid digits may be left to the tie repair, see stage_sort)
             const uint32_t d = (w[1 + p / 3] >> (kRadixBits * (p % 3))) & (kRadix - 1);
             // a warp whose 32 keys share the digit (the leading digits of clustered or pre-sorted input)
             // adds once instead of serialising 32 same-address atomics; only the hi word's digits (levels 1-10) are
@@ -523,40 +524,48 @@ cudaError_t stage_keys(Ctx* c) {
     if (e != cudaSuccess) return e;
     const uint32_t blocks = min(div_up(c->n, kKeysThreads), (uint32_t)(c->num_sms * 2));
     k_keys<<<blocks, kKeysThreads, 0, c->stream>>>(c->pos_mass, c->n, b.ctl, b.key[0][0], b.key[0][1], b.key[0][2],
-                                                   b.ghist, c->gate);
+                                                   b.ghist, sort_first_pass(c), c->gate);
     c->launches += 1;
     return cudaGetLastError();
 }
 
-// Ties of the two-word sort.  After the six passes over the mid and hi words the particles are ordered by their
-// first 20 octal digits and, inside a run of equal digits, by load index (LSD passes are stable).  Such runs are
-// cells of side 2^-20 of the root cube: with fp32 coordinates they hold one particle almost always.  The thread
-// at the head of a run of up to kTieRun particles orders it by (lo word, load index) with an insertion sort over
-// perm, sorted_pos and the lo keys; the start of a longer run is appended to a device list that k_sort_long_runs
-// works off.
+// Ties of the sort.  After the passes the particles are ordered by the leading 60 - cut bits of (hi, mid) -- cut = 0,
+// 10 or 20 low bits of the mid word are skipped with the first passes, see stage_sort -- and, inside a run of equal
+// leading bits, by load index (LSD passes are stable).  Such runs are cells of side 2^-20 (cut = 0) to 2^-13.3
+// (cut = 20) of the root cube: they hold one particle almost always, a handful in the densest part of the largest
+// systems.  The thread at the head of a run of up to kTieRun particles orders it by (low mid bits, lo word, load
+// index) with an insertion sort over perm, sorted_pos and the key words; the start of a longer run is appended to a
+// device list that k_sort_long_runs works off.
 constexpr uint32_t kTieRun = 32;
 
-__device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, const uint32_t* __restrict__ khi,
-                                          const uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
+__device__ __forceinline__ unsigned long long tie_key(uint32_t mid, uint32_t lo, uint32_t cut) {
+    return ((unsigned long long)(mid & ((1u << cut) - 1u)) << 30) | lo;
+}
+
+__device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, uint32_t cut, const uint32_t* __restrict__ khi,
+                                          uint32_t* __restrict__ kmid, uint32_t* __restrict__ klo,
                                           uint32_t* __restrict__ perm, float4* __restrict__ sorted_pos, uint32_t n,
                                           Control* __restrict__ ctl, uint32_t* __restrict__ long_start) {
     uint32_t len = 2;
-    while (i + len < n && len <= kTieRun && khi[i + len] == h && kmid[i + len] == m) ++len;
+    while (i + len < n && len <= kTieRun && khi[i + len] == h && (kmid[i + len] >> cut) == m) ++len;
     if (len > kTieRun) {
         long_start[atomicAdd(&ctl->n_long_runs, 1u)] = i;  // at most n / (kTieRun + 1) such runs
         return;
     }
-    for (uint32_t k = 1; k < len; ++k) {  // stable insertion sort by lo: equal lo keep their ascending load index
-        const uint32_t lo = klo[i + k], pk = perm[i + k];
+    for (uint32_t k = 1; k < len; ++k) {  // stable insertion sort: equal keys keep their ascending load index
+        const uint32_t lo = klo[i + k], mk = kmid[i + k], pk = perm[i + k];
+        const unsigned long long key = tie_key(mk, lo, cut);
         const float4 xk = sorted_pos[i + k];
         uint32_t j = k;
-        while (j > 0 && klo[i + j - 1] > lo) {
+        while (j > 0 && tie_key(kmid[i + j - 1], klo[i + j - 1], cut) > key) {
             klo[i + j] = klo[i + j - 1];
+            kmid[i + j] = kmid[i + j - 1];
             perm[i + j] = perm[i + j - 1];
             sorted_pos[i + j] = sorted_pos[i + j - 1];
             --j;
         }
         klo[i + j] = lo;
+        kmid[i + j] = mk;
         perm[i + j] = pk;
         sorted_pos[i + j] = xk;
     }
@@ -564,60 +573,66 @@ __device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, co
 
 // Four consecutive sorted particles per thread (16-byte loads of the hi and mid words plus one neighbour on each
 // side); a particle that ties with its successor but not with its predecessor heads a run.
-__global__ void __launch_bounds__(256) k_sort_ties(const uint32_t* __restrict__ khi, const uint32_t* __restrict__ kmid,
+__global__ void __launch_bounds__(256) k_sort_ties(const uint32_t* __restrict__ khi, uint32_t* __restrict__ kmid,
                                                    uint32_t* __restrict__ klo, uint32_t* __restrict__ perm,
                                                    float4* __restrict__ sorted_pos, uint32_t n, Control* __restrict__ ctl,
-                                                   uint32_t* __restrict__ long_start, const Gate gate) {
+                                                   uint32_t* __restrict__ long_start, const uint32_t cut, const Gate gate) {
     if (gate_closed(gate)) return;
     const uint32_t i0 = 4u * (blockIdx.x * blockDim.x + threadIdx.x);
     if (i0 >= n) return;
     uint32_t h[6], m[6];  // positions i0 - 1 .. i0 + 4; out-of-range slots get a value no key has
     if (i0 + 4 <= n) {
-        const uint4 hv = __ldg(reinterpret_cast<const uint4*>(khi + i0)), mv = __ldg(reinterpret_cast<const uint4*>(kmid + i0));
+        // (plain loads: a neighbouring thread's repair may be rewriting mid words of ITS run, never of this thread's
+        // leading bits -- a repair only permutes words whose leading bits are equal)
+        const uint4 hv = __ldg(reinterpret_cast<const uint4*>(khi + i0)), mv = *reinterpret_cast<const uint4*>(kmid + i0);
         h[1] = hv.x; h[2] = hv.y; h[3] = hv.z; h[4] = hv.w;
         m[1] = mv.x; m[2] = mv.y; m[3] = mv.z; m[4] = mv.w;
     } else {
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             h[1 + k] = (i0 + k < n) ? __ldg(&khi[i0 + k]) : 0xFFFFFFFFu;
-            m[1 + k] = (i0 + k < n) ? __ldg(&kmid[i0 + k]) : 0xFFFFFFFFu;
+            m[1 + k] = (i0 + k < n) ? kmid[i0 + k] : 0xFFFFFFFFu;
         }
     }
     h[0] = (i0 > 0) ? __ldg(&khi[i0 - 1]) : 0xFFFFFFFFu;
-    m[0] = (i0 > 0) ? __ldg(&kmid[i0 - 1]) : 0xFFFFFFFFu;
+    m[0] = (i0 > 0) ? kmid[i0 - 1] : 0xFFFFFFFFu;
     h[5] = (i0 + 4 < n) ? __ldg(&khi[i0 + 4]) : 0xFFFFFFFFu;
-    m[5] = (i0 + 4 < n) ? __ldg(&kmid[i0 + 4]) : 0xFFFFFFFFu;
+    m[5] = (i0 + 4 < n) ? kmid[i0 + 4] : 0xFFFFFFFFu;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) m[k] >>= cut;  // the leading bits the passes have sorted (0xFFFFFFFF >> cut: still no key)
 #pragma unroll
     for (int k = 1; k <= 4; ++k) {
         if (h[k] == 0xFFFFFFFFu) break;  // past the end (key words have 30 bits)
         const bool ties_next = (h[k + 1] == h[k]) && (m[k + 1] == m[k]);
         const bool ties_prev = (h[k - 1] == h[k]) && (m[k - 1] == m[k]);
-        if (ties_next && !ties_prev) sort_tie_run(i0 + k - 1, h[k], m[k], khi, kmid, klo, perm, sorted_pos, n, ctl, long_start);
+        if (ties_next && !ties_prev)
+            sort_tie_run(i0 + k - 1, h[k], m[k], cut, khi, kmid, klo, perm, sorted_pos, n, ctl, long_start);
     }
 }
 
-// Long runs of equal (hi, mid): one WARP per run (runs are taken from the list by an atomic ticket) sorts the run
-// by (lo word, position in the run) -- a stable LSD radix sort over the 30 bits of the lo word, four passes of 8-bit
-// digits on (lo, local index) pairs in scratch arrays, then one gather of perm, sorted_pos and the lo keys through the
-// resulting order.  Positions in a run ascend with the load index (the six passes are stable), so this is exactly
-// the order (key, load index) of R5.  The launch returns at once when the list is empty (every Plummer / merger
-// workload); a degenerate input -- all particles coincident, or inside one cell of side 2^-20 -- costs this kernel a
-// few milliseconds instead of costing every step a nine-pass fallback chain of empty launches.
+// Long runs of equal leading bits: one WARP per run (runs are taken from the list by an atomic ticket) sorts the run
+// by (low mid bits, lo word, position in the run) -- a stable LSD radix sort over the 30 + cut bits of that key in 8-bit
+// digits.  Only the local indices move between passes (the digit of an element is read through its index from the
+// run's own key words); one gather of perm, sorted_pos and the key words through the resulting order ends it.
+// Positions in a run ascend with the load index (the passes are stable), so this is exactly the order (key, load index)
+// of R5.  The launch returns at once when the list is empty (every Plummer / merger workload); a degenerate input --
+// all particles coincident, or a clump far smaller than the cells the passes resolve -- costs this kernel a few
+// milliseconds instead of costing every step more passes.
 struct LongRunScratch {
-    uint32_t *key_a, *key_b, *idx_a, *idx_b;  // [n] each, indexed by global position: runs are disjoint
-    uint32_t *perm_tmp, *lo_tmp;
+    uint32_t *idx_a, *idx_b;  // [n] each, indexed by global position: runs are disjoint
+    uint32_t *perm_tmp, *lo_tmp, *mid_tmp;
     float4* pos_tmp;
 };
 
 constexpr int kLongWarps = 4;
 
 __global__ void __launch_bounds__(kLongWarps * 32) k_sort_long_runs(const uint32_t* __restrict__ khi,
-                                                                    const uint32_t* __restrict__ kmid,
+                                                                    uint32_t* __restrict__ kmid,
                                                                     uint32_t* __restrict__ klo, uint32_t* __restrict__ perm,
                                                                     float4* __restrict__ sorted_pos, uint32_t n,
                                                                     Control* __restrict__ ctl,
                                                                     const uint32_t* __restrict__ long_start,
-                                                                    LongRunScratch sc, const Gate gate) {
+                                                                    LongRunScratch sc, const uint32_t cut, const Gate gate) {
     __shared__ uint32_t s_hist[kLongWarps][256];
     if (gate_closed(gate)) return;
     const uint32_t n_runs = __ldcg(&ctl->n_long_runs);
@@ -631,22 +646,23 @@ __global__ void __launch_bounds__(kLongWarps * 32) k_sort_long_runs(const uint32
         r = __shfl_sync(0xFFFFFFFFu, r, 0);
         if (r >= n_runs) break;
         const uint32_t s0 = __ldcg(&long_start[r]);
-        const uint32_t h = khi[s0], m = kmid[s0];
+        const uint32_t h = khi[s0], m = kmid[s0] >> cut;
         // length of the run: first position that leaves it
         uint32_t len = 0;
         for (uint32_t base = s0;; base += 32u) {
             const uint32_t i = base + l;
-            const bool in = i < n && khi[i] == h && kmid[i] == m;
+            const bool in = i < n && khi[i] == h && (kmid[i] >> cut) == m;
             const uint32_t out = ~__ballot_sync(0xFFFFFFFFu, in);
             if (out) { len = base - s0 + (uint32_t)(__ffs(out) - 1); break; }
         }
-        uint32_t *ka = sc.key_a + s0, *kb = sc.key_b + s0, *ia = sc.idx_a + s0, *ib = sc.idx_b + s0;
-        for (uint32_t k = l; k < len; k += 32u) { ka[k] = klo[s0 + k]; ia[k] = k; }
+        uint32_t *ia = sc.idx_a + s0, *ib = sc.idx_b + s0;
+        for (uint32_t k = l; k < len; k += 32u) ia[k] = k;
         __syncwarp();
-        for (int shift = 0; shift < 30; shift += 8) {
+        for (uint32_t shift = 0; shift < 30u + cut; shift += 8u) {
             for (int d = l; d < 256; d += 32) hist[d] = 0u;
             __syncwarp();
-            for (uint32_t k = l; k < len; k += 32u) atomicAdd(&hist[(ka[k] >> shift) & 255u], 1u);
+            for (uint32_t k = l; k < len; k += 32u)
+                atomicAdd(&hist[(uint32_t)(tie_key(kmid[s0 + k], klo[s0 + k], cut) >> shift) & 255u], 1u);
             __syncwarp();
             // exclusive scan of the 256 counts: 8 per lane, then across lanes
             uint32_t v[8], sum = 0;
@@ -667,22 +683,20 @@ __global__ void __launch_bounds__(kLongWarps * 32) k_sort_long_runs(const uint32
             for (uint32_t base = 0; base < len; base += 32u) {
                 const uint32_t k = base + l;
                 const bool valid = k < len;
-                const uint32_t key = valid ? ka[k] : 0u;
-                const uint32_t d = valid ? ((key >> shift) & 255u) : 256u + (uint32_t)l;  // invalid lanes match nobody
+                const uint32_t e = valid ? ia[k] : 0u;
+                const uint32_t d = valid ? ((uint32_t)(tie_key(kmid[s0 + e], klo[s0 + e], cut) >> shift) & 255u)
+                                         : 256u + (uint32_t)l;  // invalid lanes match nobody
                 const uint32_t peers = __match_any_sync(0xFFFFFFFFu, d);
                 uint32_t off = 0;
                 if (valid) off = hist[d];
                 __syncwarp();
                 if (valid) {
-                    const uint32_t dst = off + (uint32_t)__popc(peers & lt);
-                    kb[dst] = key;
-                    ib[dst] = ia[k];
+                    ib[off + (uint32_t)__popc(peers & lt)] = e;
                     if ((peers >> l) <= 1u) hist[d] = off + (uint32_t)__popc(peers);  // the highest peer advances the offset
                 }
                 __syncwarp();
             }
-            uint32_t* t = ka; ka = kb; kb = t;
-            t = ia; ia = ib; ib = t;
+            uint32_t* t = ia; ia = ib; ib = t;
             __threadfence_block();
             __syncwarp();
         }
@@ -690,6 +704,7 @@ __global__ void __launch_bounds__(kLongWarps * 32) k_sort_long_runs(const uint32
         for (uint32_t k = l; k < len; k += 32u) {
             sc.perm_tmp[s0 + k] = perm[s0 + k];
             sc.lo_tmp[s0 + k] = klo[s0 + k];
+            sc.mid_tmp[s0 + k] = kmid[s0 + k];
             sc.pos_tmp[s0 + k] = sorted_pos[s0 + k];
         }
         __threadfence_block();
@@ -698,6 +713,7 @@ __global__ void __launch_bounds__(kLongWarps * 32) k_sort_long_runs(const uint32
             const uint32_t src = s0 + ia[k];
             perm[s0 + k] = sc.perm_tmp[src];
             klo[s0 + k] = sc.lo_tmp[src];
+            kmid[s0 + k] = sc.mid_tmp[src];
             sorted_pos[s0 + k] = sc.pos_tmp[src];
         }
         __syncwarp();
@@ -723,8 +739,22 @@ cudaError_t sort_prepare(Ctx* c) {
     return e;
 }
 
-// The sort: six LSD passes over the mid and hi words (pass p: word mid, hi = p / 3; digit p % 3), starting from the
-// identity permutation; the outputs alternate pair buffers 1, 0, 1, 0, 1, 0, which leaves the permutation in idx[0].
+// How many of the six passes run.  The passes go over the mid word's three digits, then the hi word's; leaving out the
+// first one or two leaves particles that agree in the leading 50 or 40 key bits (cells of side 2^-16.7 / 2^-13.3 of the
+// root cube) in load order, and the tie repair after the reorder (k_sort_ties, k_sort_long_runs) puts exactly those
+// runs in order of their remaining bits -- the result is the same permutation bit for bit, whatever the choice.  What it
+// costs is the repair: measured on the Plummer sphere, 40 leading bits leave 0.3 % of the particles in runs (of 2) at
+// N = 2^15 and 17 % (runs of <= 8) at N = 2^22; 50 bits leave 0.02 % at 2^22.  The rule below keeps the expected run of
+// a Plummer core short; params.sort_passes overrides it (a strongly clustered system wants more passes).
+int sort_first_pass(const Ctx* c) {
+    if (c->prm.sort_passes) return kSortPasses - (int)c->prm.sort_passes;
+    if (c->n <= (1u << 22)) return 2;
+    if (c->n <= (1u << 25)) return 1;
+    return 0;
+}
+
+// The sort: LSD passes over the mid and hi words (pass p: word mid, hi = p / 3; digit p % 3), starting from the identity
+// permutation at pass sort_first_pass(); the starting pair buffer is chosen so that the permutation ends in idx[0].
 cudaError_t stage_sort(Ctx* c) {
     Buffers& b = c->b;
     const size_t look_entries = (size_t)div_up(c->n_max, kSortTile) * kRadix;
@@ -738,8 +768,9 @@ cudaError_t stage_sort(Ctx* c) {
     a.ticket = &b.ctl->sort_ticket;
     a.ctl = b.ctl;
     a.gate = c->gate;
-    int cur = 0;
-    for (int p = 0; p < kSortPasses; ++p) {
+    const int first = sort_first_pass(c);
+    int cur = first & 1;
+    for (int p = first; p < kSortPasses; ++p) {
         a.pass = (uint32_t)p;
         a.shift = kRadixBits * (p % 3);
         a.gbase = b.ghist + p * kRadix;
@@ -749,7 +780,7 @@ cudaError_t stage_sort(Ctx* c) {
         a.idx_in = b.idx[cur];
         a.key_out = (p == kSortPasses - 1) ? nullptr : b.pair_key[out];
         a.idx_out = b.idx[out];
-        if (p == 0) k_sort_pass<0><<<a.n_tiles, kSortThreads, kSortSmem, c->stream>>>(a);
+        if (p == first) k_sort_pass<0><<<a.n_tiles, kSortThreads, kSortSmem, c->stream>>>(a);
         else if (p % 3 == 0) k_sort_pass<2><<<a.n_tiles, kSortThreads, kSortSmem, c->stream>>>(a);
         else k_sort_pass<1><<<a.n_tiles, kSortThreads, kSortSmem, c->stream>>>(a);
         c->launches += 1;
@@ -767,18 +798,18 @@ cudaError_t stage_reorder(Ctx* c, bool write_keys) {
     return cudaGetLastError();
 }
 
-// After the reorder of a fresh sort: put the (rare) runs of equal (hi, mid) in order of their lo word -- short runs in
-// place, long ones (coincident particles, clumps far smaller than 2^-20 of the box) by k_sort_long_runs, which
-// returns at once when there are none.  Scratch of the long-run sort: the pair buffers and the load-order key words
-// (dead after the passes) and the fp64 moment array (not yet written).
+// After the reorder of a fresh sort: put the runs of equal leading key bits in order of their remaining bits -- short
+// runs in place, long ones (coincident particles, clumps far smaller than the cells the passes resolve) by
+// k_sort_long_runs, which returns at once when there are none.  Scratch of the long-run sort: the pair buffers and the
+// load-order key words (dead after the passes) and the fp64 moment array (not yet written).
 cudaError_t stage_sort_ties(Ctx* c) {
     Buffers& b = c->b;
+    const uint32_t cut = (uint32_t)(kRadixBits * sort_first_pass(c));  // low bits of the mid word the passes skipped
     k_sort_ties<<<div_up(div_up(c->n, 4), 256), 256, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
-                                                          b.ctl, b.long_start, c->gate);
-    LongRunScratch sc{b.pair_key[0], b.pair_key[1], b.idx[1], b.key[0][0], b.key[0][1], b.key[0][2],
-                      reinterpret_cast<float4*>(b.c_mom)};
+                                                          b.ctl, b.long_start, cut, c->gate);
+    LongRunScratch sc{b.pair_key[0], b.idx[1], b.key[0][0], b.key[0][1], b.key[0][2], reinterpret_cast<float4*>(b.c_mom)};
     k_sort_long_runs<<<c->num_sms, kLongWarps * 32, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
-                                                                 b.ctl, b.long_start, sc, c->gate);
+                                                                 b.ctl, b.long_start, sc, cut, c->gate);
     c->launches += 2;
     return cudaGetLastError();
 }

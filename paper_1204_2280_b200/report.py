@@ -218,17 +218,97 @@ def issue_mix(reps: int) -> dict:
             "scheduler_cycles_per_round": measure_issue_mix(40000)}
 
 
+def markdown(doc: dict) -> str:
+    """The tables of profiles/r2_configs.md from the dictionary main() prints (`--markdown FILE`)."""
+    o = ["# The BASELINE.json configurations that are not the bench line\n",
+         "Command: `python -m paper_1204_2280_b200.report --markdown FILE > FILE.json`.  One B200, seeded Plummer spheres, "
+         "CUDA-event stage times of the library (median of 5), L2 not flushed between repetitions.\n"]
+    if "theta_sweep" in doc:
+        d = doc["theta_sweep"]
+        o += [f"## configs[1]: N = {d['n']}, eps = {d['eps']}, theta sweep\n",
+              "| theta | p-p per particle | p-c per particle | walk ms | step ms |", "|---|---|---|---|---|"]
+        o += [f"| {th} | {r['pp_per_particle']:.0f} | {r['pc_per_particle']:.0f} | {r['walk_ms']:.3f} | {r['step_ms']:.3f} |"
+              for th, r in d["by_theta"].items()]
+        o.append("")
+    if "leapfrog" in doc:
+        d = doc["leapfrog"]
+        o += [f"## configs[2]: N = {d['n']}, eps = {d['eps']}, {d['steps']} KDK steps, dt = {d['dt']}, tree rebuilt every step "
+              "(bonsai_leapfrog_step, graph replay)\n",
+              "| theta | ms per step | particle-steps per s | relative energy drift over the run |", "|---|---|---|---|"]
+        o += [f"| {th} | {r['ms_per_step']:.3f} | {r['particle_steps_per_s']:.3e} | {r['rel_energy_drift_8_steps']:.2e} |"
+              for th, r in d["by_theta"].items()]
+        o.append("")
+    if "block_step" in doc:
+        d = doc["block_step"]
+        o += [f"## configs[4]: N = {d['n']}, theta = {d['theta']}, full rebuild, walk of an active subset (P:L32)\n",
+              f"Full walk {d['full_walk_ms']:.3f} ms; stages before the walk {d['full_pre_walk_ms']:.3f} ms.\n",
+              "| subset | walk ms | groups stage ms | walk-time reduction | N / N_active |", "|---|---|---|---|---|"]
+        o += [f"| {k} | {r['walk_ms']:.4f} | {r['groups_ms']:.3f} | {r['walk_time_reduction']:.1f} x | {r['ideal']} |"
+              for k, r in d["subsets"].items()]
+        r = d.get("refreshed_clustered_N/16")
+        if r:
+            o.append(f"\nRefreshed tree (bonsai_refresh_tree, R25) instead of a rebuild, clustered N/16: reorder "
+                     f"{r['reorder_ms']:.3f} + groups {r['groups_ms']:.3f} + multipoles {r['multipoles_ms']:.3f} + walk "
+                     f"{r['walk_ms']:.3f} = {r['step_ms']:.3f} ms against {r['rebuild_step_ms']:.3f} ms with a rebuild.")
+        o.append("")
+    if "scaling" in doc:
+        names = ("bbox", "keys", "sort", "reorder", "build", "groups", "multipoles", "walk")
+        o += ["## Scaling with N (the paper's Fig. 2 quantity, P:L48), theta = 0.75\n",
+              "| N | " + " | ".join(names) + " | stage sum ms | step ms, graph replay | step ms, kernel by kernel | "
+              "particles/s (graph) | walk share |", "|---|" + "---|" * (len(names) + 5)]
+        for r in doc["scaling"].values():
+            o.append(f"| {r['n']} | " + " | ".join(f"{r['stage_ms'][k]:.3f}" for k in names) +
+                     f" | {r['step_ms']:.3f} | {r['step_ms_graph']:.3f} | {r.get('step_ms_no_graph', float('nan')):.3f} | "
+                     f"{r['n'] / r['step_ms_graph'] * 1e3:.3e} | {100 * r['walk_share']:.0f} % |")
+        o.append("")
+    if "merger" in doc:
+        d = doc["merger"]["by_workload"]
+        m, pl = d["merger"], d["plummer"]
+        o += [f"## Second workload (row f4): two Plummer spheres, mass ratio 3, on approach, N = {doc['merger']['n']}\n",
+              f"merger {m['step_ms']:.3f} ms per step ({m['n_cells']} cells, {m['n_groups']} groups, {m['pp_per_particle']:.0f} p-p + "
+              f"{m['pc_per_particle']:.0f} p-c per particle) against {pl['step_ms']:.3f} ms for the single sphere "
+              f"({pl['n_cells']} cells, {pl['n_groups']} groups).\n"]
+    if "mac" in doc:
+        d = doc["mac"]
+        o += [f"## Row f3: MAC variants, N = {d['n']} (error of {d['sinks_compared']} sinks against: {d['error_reference']})\n",
+              "| variant | theta | median force error | 99th percentile | p-p per particle | p-c per particle | walk ms |",
+              "|---|---|---|---|---|---|---|"]
+        for name, by in d["variants"].items():
+            o += [f"| {name} | {th} | {r['acc_err_median']:.2e} | {r['acc_err_p99']:.2e} | {r['pp_per_particle']:.0f} | "
+                  f"{r['pc_per_particle']:.0f} | {r['walk_ms']:.3f} |" for th, r in by.items()]
+        o.append("")
+    if "issue_mix" in doc:
+        d = doc["issue_mix"]
+        o += ["## Microbenchmarks behind the walk's issue-slot budget (csrc/peak.cu)\n", "| measurement | result |", "|---|---|"]
+        o += [f"| FP32 peak, {k} | {v:.2f} TFLOP/s |" for k, v in d["fp32_peak_tflops"].items()]
+        o += [f"| scheduler cycles per round, {k} | {v:.2f} |" for k, v in d["scheduler_cycles_per_round"].items()]
+        o.append("")
+    return "\n".join(o)
+
+
 def main() -> None:
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--reps", type=int, default=5)
     ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling", "merger", "mac", "issue_mix"), default=None)
+    ap.add_argument("--markdown", default=None, help="also write the tables as markdown to this file")
+    ap.add_argument("--from-json", dest="from_json", default=None,
+                    help="render --markdown from an earlier JSON output instead of measuring (needs no GPU)")
     args = ap.parse_args()
+    if args.from_json:
+        with open(args.from_json) as f:
+            text = f.read()
+        with open(args.markdown, "w") as f:
+            f.write(markdown(json.loads(text[text.index("{"):])))
+        return
     if not torch.cuda.is_available():
         raise SystemExit("report: no CUDA device -- libbonsai has no CPU fallback")
     parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "scaling": scaling,
              "merger": merger, "mac": mac_variants, "issue_mix": issue_mix}
     doc = {k: f(args.reps) for k, f in parts.items() if args.only in (None, k)}
     print(json.dumps(doc, indent=1))
+    if args.markdown:
+        with open(args.markdown, "w") as f:
+            f.write(markdown(doc))
 
 
 if __name__ == "__main__":
