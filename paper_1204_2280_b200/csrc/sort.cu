@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, ui
 //   t = x - lo;  u = t * (2^30 / side);  i = trunc(u) clamped to [0, 2^30 - 1].
 // Octal digit of level L (1..30) = 4 x_bit + 2 y_bit + z_bit at bit 30 - L; words hi/mid/lo hold levels
 // 1-10 / 11-20 / 21-30.  Grid-stride, 16 B in, 3 x 4 B out, all coalesced.  The same pass builds the
-// digit histograms of all six sort passes in shared memory (a histogram does not depend on the order
+// digit histograms of the sort passes that will run in shared memory (a histogram does not depend on the order
 // of the keys, so the sort never has to count again).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t spread10(uint32_t v) {  // 10 bits -> every third bit of 30
@@ -229,10 +229,11 @@ __global__ void __launch_bounds__(kRadix) k_sort_gscan(uint32_t* __restrict__ gh
 // 30-bit word, index) PAIRS: a pass reads 8 B and writes 8 B per particle.  When the passes of one word are
 // done the next word is fetched through the index (gather from the load-order key arrays); the sorted
 // 90-bit keys are re-derived from the reordered positions in k_reorder (a key is a pure function of the
-// position and the root cube).  The sort runs SIX passes, over the mid and hi words: the lo word
-// (levels 21-30) almost never decides the order; the runs of equal (hi, mid) are put in order after the
-// reorder, short ones in place by k_sort_ties, long ones (coincident particles, clumps far smaller than
-// 2^-20 of the box) by k_sort_long_runs (see stage_sort_ties).
+// position and the root cube).  The sort runs FOUR to SIX passes, over the leading 40 to 60 bits of the
+// mid and hi words (by size, see sort_first_pass): the remaining bits almost never decide the order; the
+// runs of equal leading bits are put in order after the reorder, short ones in place by k_sort_ties, long
+// ones (coincident particles, clumps far smaller than the cells the passes resolve) by k_sort_long_runs
+// (see stage_sort_ties).
 //
 // One kernel per pass, single sweep with decoupled look-back:
 //   * tiles of kSortTile pairs are handed out by an atomic ticket, so a tile's predecessors have
@@ -552,9 +553,15 @@ __device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, ui
         long_start[atomicAdd(&ctl->n_long_runs, 1u)] = i;  // at most n / (kTieRun + 1) such runs
         return;
     }
+    unsigned long long top = tie_key(kmid[i], klo[i], cut);  // largest key of the sorted prefix [i, i + k)
     for (uint32_t k = 1; k < len; ++k) {  // stable insertion sort: equal keys keep their ascending load index
-        const uint32_t lo = klo[i + k], mk = kmid[i + k], pk = perm[i + k];
+        const uint32_t lo = klo[i + k], mk = kmid[i + k];
         const unsigned long long key = tie_key(mk, lo, cut);
+        if (key >= top) {  // already in place (half of the runs of two): nothing else of this particle is touched
+            top = key;
+            continue;
+        }
+        const uint32_t pk = perm[i + k];
         const float4 xk = sorted_pos[i + k];
         uint32_t j = k;
         while (j > 0 && tie_key(kmid[i + j - 1], klo[i + j - 1], cut) > key) {

@@ -19,7 +19,15 @@ def main(path):
         print(f"| {r['test']} | {r['n']} | {r.get('theta', '')} | {r.get('sinks_sampled', r.get('n_checked'))} | "
               f"{r['count_frac']:.6f} | {r['n_borderline_mismatch']} | {r['acc_max']:.2e} | {r['acc_med']:.2e} | "
               f"{r['pot_max']:.2e} | {r['pot_med']:.2e} |")
+    deep = [r for r in walk if r.get("deep_tree")]
+    walk = [r for r in walk if not r.get("deep_tree")]
     rest = [r for r in walk if r["test"] in ("check_walk", "check_walk_sampled")]
+    if deep:
+        print(f"\nClumps far below the 13th level (sort-pass tests, {len(deep)} calls, trees up to 26 levels deep): one "
+              f"ulp(fp32) of a centre-of-mass coordinate is 1e-3 of a cell side there, so opening tests outside the oracle's "
+              f"borderline margin may flip; required instead: counts identical for >= 98 % of the sinks (lowest "
+              f"{min(r['count_frac'] for r in deep):.5f}, {sum(r['n_borderline_mismatch'] for r in deep)} mismatching "
+              f"sinks in total) and every mismatching sink within 1e-2 of the oracle.")
     if rest:
         print(f"\nAll other walk comparisons ({len(rest)} calls, N = {min(r['n'] for r in rest)} .. {max(r['n'] for r in rest)}): "
               f"lowest identical-count fraction {min(r['count_frac'] for r in rest):.5f}, "

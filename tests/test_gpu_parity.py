@@ -165,7 +165,7 @@ def check_walk(b: Bonsai, out, ref: O.Step, active=None, count_frac=0.999, eps=N
         assert eb.max() <= BORDER_MAX and epb.max() <= BORDER_MAX, (eb.max(), epb.max())
     stats = dict(n=int(n), n_checked=int(sel.sum()), count_frac=float(frac), acc_max=float(ea.max()),
                  acc_med=float(np.median(ea)), pot_max=float(ep.max()), pot_med=float(np.median(ep)),
-                 n_borderline_mismatch=int(diff.sum()))
+                 n_borderline_mismatch=int(diff.sum()), deep_tree=bool(deep_tree))
     record(tag or "check_walk", **stats)
     return stats
 
