@@ -79,11 +79,16 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_levels(const uint32_t* __
         uint32_t mask = 0;
         if (i < n) {
             const int j = (int)(i - base) + H;  // s_lcp index of boundary i
+            // candidate start b = i - nleaf + 1 + t, candidate ends (i, b + nleaf].  No range checks: boundaries outside
+            // [0, n] read -1 like boundaries 0 and n themselves, so an end past n repeats what the end n already
+            // contributed, and a start before 0 sees fewer ends than the start 0 that is then a candidate too.
             int best = 127, rmin = 127;
+            const int8_t* lo_side = &s_lcp[j - nleaf + 1];
+            const int8_t* hi_side = &s_lcp[j + 1];
+#pragma unroll 8
             for (int t = 0; t < nleaf; ++t) {
-                const long long b = (long long)i - nleaf + 1 + t;  // candidate start, candidate end = b + nleaf
-                if (b + nleaf <= (long long)n) rmin = min(rmin, (int)s_lcp[j + 1 + t]);
-                if (b >= 0) best = min(best, max((int)s_lcp[j - nleaf + 1 + t], rmin));
+                rmin = min(rmin, (int)hi_side[t]);
+                best = min(best, max((int)lo_side[t], rmin));
             }
             const int ll = min(best + 1, kMaxLevel);
             leaf_level[i] = (int8_t)ll;
