@@ -553,15 +553,11 @@ __device__ __noinline__ void sort_tie_run(uint32_t i, uint32_t h, uint32_t m, ui
         long_start[atomicAdd(&ctl->n_long_runs, 1u)] = i;  // at most n / (kTieRun + 1) such runs
         return;
     }
-    unsigned long long top = tie_key(kmid[i], klo[i], cut);  // largest key of the sorted prefix [i, i + k)
+    // (skipping the loads of perm / sorted_pos for particles that are already in place was measured: 45.6 against
+    // 39.5 us at N = 2^22 -- the extra compare chain costs more than the loads it saves)
     for (uint32_t k = 1; k < len; ++k) {  // stable insertion sort: equal keys keep their ascending load index
-        const uint32_t lo = klo[i + k], mk = kmid[i + k];
+        const uint32_t lo = klo[i + k], mk = kmid[i + k], pk = perm[i + k];
         const unsigned long long key = tie_key(mk, lo, cut);
-        if (key >= top) {  // already in place (half of the runs of two): nothing else of this particle is touched
-            top = key;
-            continue;
-        }
-        const uint32_t pk = perm[i + k];
         const float4 xk = sorted_pos[i + k];
         uint32_t j = k;
         while (j > 0 && tie_key(kmid[i + j - 1], klo[i + j - 1], cut) > key) {

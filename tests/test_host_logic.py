@@ -36,6 +36,34 @@ def test_library_exports_every_declared_symbol():
     assert lib.bonsai_strerror(-2) == b"call out of order"
 
 
+def test_parameter_validation_needs_no_gpu():
+    """bonsai_workspace_bytes resolves and checks bonsai_params on the host (0 = rejected): the defaults, the kernel
+    choices added in round 2 (sort_passes in {0, 4, 5, 6}, mult_kernel in {0, 1, 2}) and the older limits."""
+    import ctypes
+    from paper_1204_2280_b200 import build as B
+    from paper_1204_2280_b200.bonsai import Params
+    lib = ctypes.CDLL(B.build())
+    lib.bonsai_workspace_bytes.restype = ctypes.c_size_t
+    lib.bonsai_workspace_bytes.argtypes = [ctypes.c_uint32, ctypes.POINTER(Params)]
+
+    def nbytes(n=100_000, **kw):
+        p = Params()
+        for k, v in kw.items():
+            setattr(p, k, v)
+        return lib.bonsai_workspace_bytes(n, ctypes.byref(p))
+
+    base = nbytes()
+    assert base > 100_000 * 100 and base == lib.bonsai_workspace_bytes(100_000, None)
+    for passes in (4, 5, 6):
+        assert nbytes(sort_passes=passes) == base          # a launch choice, not a layout choice
+    for bad in (1, 3, 7):
+        assert nbytes(sort_passes=bad) == 0
+    assert nbytes(mult_kernel=1) == base and nbytes(mult_kernel=2) == base and nbytes(mult_kernel=3) == 0
+    assert nbytes(nleaf=65) == 0 and nbytes(ncrit=65) == 0 and nbytes(group_mode=3) == 0
+    assert nbytes(mac_mode=2) == 0 and nbytes(order=3) == 0 and nbytes(rebuild_factor=0.5) == 0
+    assert nbytes(n=0) == 0
+
+
 _WORKER = r"""
 import os, sys
 sys.path.insert(0, {root!r})
