@@ -423,7 +423,7 @@ def run_ours(args):
 
 
 # Algorithmic bytes per particle of the HBM-bound stages (SURVEY.md section 8(d) floors):
-#   keys: 16 in + 3 key words out; sort: P pair passes (P = 4 up to n = 2^22, 5 up to 2^25, else 6: the library's rule,
+#   keys: 16 in + 3 key words out; sort: P pair passes (P = 4 up to n = 2^23, 5 up to 2^25, else 6: the library's rule,
 #   csrc/sort.cu sort_first_pass) x (8 in + 8 out), minus the index read of the first pass (iota) and the key write of
 #   the last; reorder: perm + record in, record + 3 key words out,
 #   plus the tie check re-reading the hi and mid words; build: the single-pass floor, 12 (keys once) + 4 (cell
@@ -431,7 +431,7 @@ def run_ours(args):
 #   x 48 B out + the children's records re-read by the internal cells (~0.05 x 48 B) = 30.
 def sort_passes(a):
     n = _workload(a.workload)[1]
-    return 4 if n <= (1 << 22) else 5 if n <= (1 << 25) else 6
+    return 4 if n <= (1 << 23) else 5 if n <= (1 << 25) else 6
 
 
 ALG_BYTES = {

@@ -76,7 +76,7 @@ typedef struct {
                             arrive climbs (small systems), 2 = tiles of cells deepest first, parents wait            */
     uint32_t sort_passes;/* [0] radix passes of the key sort (a2): 4, 5 or 6 passes of 10 bits over the leading 40, 50 or 60
                             key bits; particles that agree in those are put in order of their remaining bits after the
-                            reorder (the permutation is the same bit for bit).  0 = by size: 4 up to n = 2^22, 5 up to
+                            reorder (the permutation is the same bit for bit).  0 = by size: 4 up to n = 2^23, 5 up to
                             2^25, else 6 (a strongly clustered system wants more passes)                             */
 } bonsai_params;
 
