@@ -258,6 +258,35 @@ int bonsai_leapfrog_step(bonsai_ctx* ctx, float* pos_mass_dev, float* vel_dev, f
 int bonsai_diagnostics(bonsai_ctx* ctx, const float* pos_mass_dev, const float* vel_dev, const float* acc_pot_dev,
                        uint32_t n, double* out12_dev);
 
+/* The same diagnostics (R24; the 12 sums documented at bonsai_diagnostics) for callers that CANNOT ALLOCATE device
+ * memory: no context, no workspace.  bonsai_diagnostics() is only reachable through a context, and a context wants a
+ * workspace of several hundred bytes per particle from the caller; a monitor that is hooked into a running
+ * simulation whose memory pool is spent, a plug-in whose host forbids cudaMalloc, or a loop that must avoid the
+ * device-wide synchronisation cudaMalloc / cudaFree can cause, has no such buffer to give.  This call needs only the
+ * three particle arrays and the result buffer.  Its scratch (block partials + a ticket) is a fixed array inside the
+ * library image:
+ *     BONSAI_DIAG_STATIC_SCRATCH_BYTES = 113 920 bytes of device memory, held on EVERY GPU that loads libbonsai,
+ *     from load until the process exits, used or not.
+ * The call allocates nothing, on the host or on the device (no cudaMalloc / cudaFree / allocating library routine).
+ *   pos_mass_dev, vel_dev, acc_pot_dev   device float4[n], 16-byte aligned, caller-owned, read only
+ *   n            1 .. BONSAI_DIAG_STATIC_MAX_N (2^30, the ceiling bonsai_create puts on n_max; the kernel's 32-bit
+ *                strided index is safe up to there).  Larger n, like n = 0, is refused with BONSAI_EINVAL before any
+ *                CUDA call is made; the scratch itself (1184 rows, the grid cap) serves every n up to the limit.
+ *   out12_dev    device double[12], 8-byte aligned, caller-owned, written by the kernel
+ *   cuda_stream  a cudaStream_t of the CURRENT device (NULL = legacy default stream); asynchronous on it
+ * Sharing.  All calls on a device share the one array and it keeps the last call's contents; the ticket is cleared on
+ * the stream before each launch, the rows are rewritten before they are read.  Calls that may run on the GPU at the
+ * same time (two streams, two threads) RACE on it and return wrong sums: keep them on one stream or order them
+ * yourself.  Calls on different devices do not interfere.
+ * First call.  The first call on each device resolves the array's device address (with that device current) and may
+ * load the module while doing so; issue it once per device before any stream capture begins.
+ * Result.  Same grid rule and summation order as bonsai_diagnostics(); deterministic for a given n.
+ * EINVAL (null / misaligned / n out of range), ECUDA. */
+#define BONSAI_DIAG_STATIC_MAX_N          (1u << 30)
+#define BONSAI_DIAG_STATIC_SCRATCH_BYTES  113920u
+int bonsai_diagnostics_static(const float* pos_mass_dev, const float* vel_dev, const float* acc_pot_dev, uint32_t n,
+                              double* out12_dev, void* cuda_stream);
+
 /* ---- Block time-steps (R26, R27; "block time-step algorithm", "N_active") -----------------
  * The paper states no criterion or scheme.  R26: particle i steps with dt_i = dt_max 2^-k_i, its rung k_i in
  * [0, kmax] the smallest k with dt_max 2^-k <= eta sqrt(eps / |a_i|) (fp64 on the fp32 acceleration).  Time is

@@ -32,7 +32,7 @@ SYMBOLS = (
     "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
     "bonsai_timestep_rungs", "bonsai_active_mask", "bonsai_kick_rungs", "bonsai_block_tick",
     "bonsai_measure_fp32_peak", "bonsai_get_rebuild_stats", "bonsai_step", "bonsai_get_graph_replays",
-    "bonsai_measure_issue_mix",
+    "bonsai_measure_issue_mix", "bonsai_diagnostics_static",
 )
 
 
@@ -106,6 +106,7 @@ def lib() -> C.CDLL:
     L.bonsai_drift.argtypes = [vp, vp, vp, u32, f32]
     L.bonsai_leapfrog_step.argtypes = [vp, vp, vp, vp, u32, f32, f32, f32]
     L.bonsai_diagnostics.argtypes = [vp, vp, vp, vp, u32, vp]
+    L.bonsai_diagnostics_static.argtypes = [vp, vp, vp, u32, vp, vp]
     L.bonsai_get_rebuild_stats.argtypes = [vp, C.POINTER(u32), C.POINTER(u32), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.bonsai_measure_issue_mix.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
     L.bonsai_measure_fp32_peak.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
@@ -134,6 +135,40 @@ def measure_fp32_peak(packed: bool = True, iters: int = 20000, stream: "torch.cu
     st = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
     _check(lib().bonsai_measure_fp32_peak(st, int(bool(packed)), int(iters), C.byref(out)), "bonsai_measure_fp32_peak")
     return float(out.value)
+
+
+DIAG_STATIC_MAX_N = 1 << 30            # BONSAI_DIAG_STATIC_MAX_N
+DIAG_STATIC_SCRATCH_BYTES = 113920     # BONSAI_DIAG_STATIC_SCRATCH_BYTES
+
+
+def diagnostics_static(pos_mass: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor, out: torch.Tensor,
+                       stream: "torch.cuda.Stream | None" = None) -> torch.Tensor:
+    """bonsai_diagnostics_static: the 12 diagnostics sums (DIAG_FIELDS) without a context or a workspace.
+
+    For code that cannot allocate device memory (a monitor inside a simulation whose memory pool is spent, a plug-in
+    whose host forbids cudaMalloc, a loop that must not risk the device-wide synchronisation of cudaMalloc / cudaFree):
+    the scratch is a fixed 113 920-byte array inside libbonsai, held on every GPU that loads the library.  This wrapper
+    allocates nothing either, which is why ``out`` (float64[12] on the tensors' device) is a required argument.
+    All calls on a device share that scratch: keep them on one stream -- calls that overlap on the GPU race.  The first
+    call on a device resolves the scratch address and should come before any stream capture.  n <= DIAG_STATIC_MAX_N."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
+    n = int(pos_mass.shape[0])
+    if n > DIAG_STATIC_MAX_N:
+        raise ValueError(f"bonsai_diagnostics_static: n = {n} exceeds BONSAI_DIAG_STATIC_MAX_N = {DIAG_STATIC_MAX_N}")
+    for t in (pos_mass, vel, acc_pot):
+        if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == (n, 4)
+                and t.device == pos_mass.device):
+            raise ValueError("bonsai_diagnostics_static: contiguous float32 CUDA tensors of shape (n, 4) on one device")
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 12
+            and out.device == pos_mass.device):
+        raise ValueError("bonsai_diagnostics_static: out must be a contiguous float64[12] tensor on the same device")
+    with torch.cuda.device(pos_mass.device):  # the device that owns the buffers and the stream must be current
+        st = C.c_void_p(stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream)
+        _check(lib().bonsai_diagnostics_static(C.c_void_p(pos_mass.data_ptr()), C.c_void_p(vel.data_ptr()),
+                                               C.c_void_p(acc_pot.data_ptr()), n, C.c_void_p(out.data_ptr()), st),
+               "bonsai_diagnostics_static")
+    return out
 
 
 def measure_issue_mix(iters: int = 20000) -> dict:
