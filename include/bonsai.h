@@ -134,7 +134,8 @@ int bonsai_walk(bonsai_ctx* ctx, float theta, float eps, const uint8_t* active_m
  * from then on (the four most recent combinations are kept): below ~10^5 particles a step is bound by launch gaps
  * (P:L32).  The replay enqueues exactly the kernels of the staged calls; results are bit-identical.  The graph reads
  * the buffers, not a snapshot of them: new particle data in the same buffers needs no new capture.  A caller that
- * passes different buffers on every call gains nothing (16 misses in a row switch capturing off for the context).
+ * passes different buffers on every call gains nothing (after 16 misses in a row the next 256 calls are enqueued kernel
+ * by kernel, then capturing is tried again).
  * EINVAL / ESTATE / ECUDA as the staged calls. */
 int bonsai_step(bonsai_ctx* ctx, const float* pos_mass_dev, uint32_t n, float theta, float eps,
                 const uint8_t* active_mask_dev, float* acc_pot_dev_out);
@@ -328,7 +329,8 @@ int bonsai_get_rebuild_stats(bonsai_ctx* ctx, uint32_t* n_decisions, uint32_t* n
 
 /* Per-stage device times.  bonsai_set_timing(ctx, 1) records CUDA events around every stage from then on;
  * bonsai_get_stage_ms() waits for the stream and writes, per stage, the milliseconds SUMMED over its executions
- * since the previous bonsai_get_stage_ms() (or bonsai_set_timing) call -- up to 8 executions per stage:
+ * since the previous bonsai_get_stage_ms() (or bonsai_set_timing) call (any number of executions; every 9th execution of a
+ * stage waits for the previous eight to fold their times into a host-side sum):
  * 0 bbox, 1 keys, 2 sort, 3 reorder, 4 build, 5 groups, 6 multipoles, 7 walk, 8 integrate (kicks, drifts). */
 int bonsai_set_timing(bonsai_ctx* ctx, int enable);
 int bonsai_get_stage_ms(bonsai_ctx* ctx, float out_ms[BONSAI_N_STAGES]);

@@ -115,27 +115,40 @@ size_t carve(unsigned char* base, uint32_t n, const bonsai_params& p, Buffers* b
     t.host_out = cv.take<float4>(n);
     t.host_mask = cv.take<uint8_t>(n);
     t.tick_mask = cv.take<uint8_t>(n);
+    t.tie_pos = cv.take<float4>(n);
     if (b) *b = t;
     return (cv.off + kAlign - 1) / kAlign * kAlign;
 }
 
 // One timed interval of a stage.  A stage may run several times between two bonsai_get_stage_ms() calls (the
 // groups in bonsai_build_tree and again in a masked bonsai_walk, the kicks of a tick): every run takes the next
-// event pair of the stage and bonsai_get_stage_ms() sums them; beyond kStageIntervals the last pair is re-used.
+// event pair of the stage and bonsai_get_stage_ms() sums them; when all kStageIntervals pairs are in use the next run
+// first folds them into Ctx::ms_acc (a host wait on the last pair) and starts over.
 struct StageTimer {
     Ctx* c;
     int stage, slot;
     StageTimer(Ctx* c_, int s) : c(c_), stage(s), slot(0) {
         if (c->timing) {
-            slot = c->ev_count[stage] < kStageIntervals ? c->ev_count[stage] : kStageIntervals - 1;
+            if (c->ev_count[stage] == kStageIntervals) fold();
+            slot = c->ev_count[stage];
             cudaEventRecord(c->ev[stage][slot][0], c->stream);
         }
     }
     ~StageTimer() {
         if (c->timing) {
             cudaEventRecord(c->ev[stage][slot][1], c->stream);
-            if (c->ev_count[stage] < kStageIntervals) c->ev_count[stage] += 1;
+            c->ev_count[stage] += 1;
         }
+    }
+    // every event pair of this stage is in use: wait for the last one, add the intervals to the host-side sum and start
+    // over with the first pair, so that no interval is lost (timing mode only; this is the one place a stage call waits)
+    void fold() {
+        cudaEventSynchronize(c->ev[stage][kStageIntervals - 1][1]);
+        for (int i = 0; i < kStageIntervals; ++i) {
+            float ms = 0.0f;
+            if (cudaEventElapsedTime(&ms, c->ev[stage][i][0], c->ev[stage][i][1]) == cudaSuccess) c->ms_acc[stage] += ms;
+        }
+        c->ev_count[stage] = 0;
     }
 };
 
@@ -205,6 +218,8 @@ int bonsai_create(uint32_t n_max, const bonsai_params* params, void* workspace_d
     c.ev_fork = c.ev_join = nullptr;
     c.graph_clock = c.graph_replays = 0;
     c.graph_misses = 0;
+    c.graph_pause = 0;
+    for (int s = 0; s < BONSAI_N_STAGES; ++s) c.ms_acc[s] = 0.0;
     for (int k = 0; k < kGraphSlots; ++k) c.graphs[k].valid = false;
     // kernel attributes and occupancy are per device: set for every context (idempotent), never behind a
     // process-wide flag
@@ -311,6 +326,7 @@ static int build_tree_and_multipoles(Ctx* c) {
 // sequences are enqueued behind opposite gates on Control::rebuild_flag; there is no host read-back.
 static int build_or_refresh_on_device(Ctx* c) {
     BONSAI_TRY(stage_rebuild_decide(c, c->prm.rebuild_factor));
+    BONSAI_TRY(stage_recover(c));  // a set status made the decision "rebuild" (policy.cu): as every build, clear it first
     Buffers& b = c->b;
     c->gate = Gate{&b.ctl->rebuild_flag, 1u};
     int rc = build_chain(c);
@@ -403,9 +419,15 @@ int run_sequence(bonsai_ctx* h, const GraphKey& key, F&& enqueue) {
         }
     }
     // a caller that passes fresh buffers every call would pay a capture + instantiation each time: after 16 misses in
-    // a row the context stops capturing
+    // a row the next kGraphPause calls are enqueued directly (no look-up of new keys, no capture), then capturing is
+    // tried again -- a caller whose arguments settle later gets its graphs back
+    if (c->graph_pause > 0) {
+        c->graph_pause -= 1;
+        return enqueue();
+    }
     if (++c->graph_misses > 16) {
-        c->prm.no_graph = 1;
+        c->graph_misses = 0;
+        c->graph_pause = kGraphPause;
         return enqueue();
     }
     if (!c->capture_stream && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
@@ -766,7 +788,7 @@ int bonsai_set_timing(bonsai_ctx* h, int enable) {
                     if (cudaEventCreate(&c.ev[s][i][k]) != cudaSuccess) return BONSAI_ECUDA;
     }
     c.timing = enable != 0;
-    for (int s = 0; s < BONSAI_N_STAGES; ++s) c.ev_count[s] = 0;
+    for (int s = 0; s < BONSAI_N_STAGES; ++s) { c.ev_count[s] = 0; c.ms_acc[s] = 0.0; }
     return BONSAI_OK;
 }
 
@@ -775,7 +797,8 @@ int bonsai_get_stage_ms(bonsai_ctx* h, float out_ms[BONSAI_N_STAGES]) {
     Ctx& c = h->c;
     if (cudaStreamSynchronize(c.stream) != cudaSuccess) return BONSAI_ECUDA;
     for (int s = 0; s < BONSAI_N_STAGES; ++s) {
-        out_ms[s] = 0.0f;
+        out_ms[s] = (float)c.ms_acc[s];
+        c.ms_acc[s] = 0.0;
         for (int i = 0; i < c.ev_count[s]; ++i) {
             float ms = 0.0f;
             if (cudaEventElapsedTime(&ms, c.ev[s][i][0], c.ev[s][i][1]) != cudaSuccess) return BONSAI_ECUDA;

@@ -32,6 +32,7 @@ constexpr int kLevelSlots = 32;                       // levels 0..30, padded
 constexpr int kMaxNleaf = 64;
 
 constexpr int kBboxMaxBlocks = 2048;       // rows of bbox_partial; stage_bbox clamps its grid to this
+constexpr uint32_t kGraphPause = 256;      // calls enqueued directly after 16 graph misses in a row
 constexpr int kStageIntervals = 8;         // event pairs per stage: a stage that runs several times between two
                                            // bonsai_get_stage_ms() calls (groups in build and in a masked walk, the
                                            // kicks of a tick) is summed over its intervals
@@ -144,6 +145,7 @@ struct Buffers {
     double* diag_partial;      // [kDiagMaxBlocks][12] block partials of k_diagnostics
     // staging of bonsai_step_host
     float4 *host_in, *host_out;
+    float4* tie_pos;           // [n] scratch of k_sort_long_runs: a run's particles while they are permuted
     uint8_t* host_mask;
     uint8_t* tick_mask;        // [n] active mask of bonsai_block_tick
 };
@@ -194,7 +196,8 @@ struct Ctx {
     bool tree_refreshed;       // positions were re-gathered into a frozen tree: multipoles take l from the extents (R25)
     bool timing;
     cudaEvent_t ev[BONSAI_N_STAGES][kStageIntervals][2];
-    int ev_count[BONSAI_N_STAGES];  // intervals recorded since the last bonsai_get_stage_ms()
+    int ev_count[BONSAI_N_STAGES];  // intervals recorded since the last bonsai_get_stage_ms() or fold
+    double ms_acc[BONSAI_N_STAGES]; // ms of the intervals already folded (a stage ran more than kStageIntervals times)
     uint64_t launches;
     int num_sms;
     int device;                // the CUDA device the context was created on
@@ -203,7 +206,8 @@ struct Ctx {
     cudaEvent_t ev_fork, ev_join; // fork / join of that branch (no timing)
     GraphSlot graphs[kGraphSlots];
     uint64_t graph_clock, graph_replays;
-    uint32_t graph_misses;     // consecutive calls that found no captured graph (16 in a row switch capturing off)
+    uint32_t graph_misses;     // consecutive calls that found no captured graph (16 in a row pause capturing)
+    uint32_t graph_pause;      // calls left to enqueue directly before capturing is tried again
     Gate gate;                 // applied to every launch of the build chain (bbox .. tree) while it is set (R30)
     bool tree_auto;            // the tree on the device was rebuilt OR refreshed by a device-side decision (R30)
     int walk_blocks_per_sm[8]; // occupancy of the k_walk instances on this device (set in bonsai_create)

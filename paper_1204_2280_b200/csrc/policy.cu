@@ -6,6 +6,10 @@
 //   I_ref = I of the first recorded walk after the last full build
 //   at the start of a tick:  rebuild  <=>  a reference exists  and  I_last > factor I_ref      (fp64, factor fp32)
 //
+// Outside the method: a tick that finds the sticky device status set (cell capacity or walk stack overflow in an
+// earlier tick) rebuilds whatever the totals say -- only a build clears the status (k_recover), and with the status set
+// the multipole pass and the walk return at once, so a refreshed tick would silently compute nothing.
+//
 // The decision is taken ON THE DEVICE (the totals of the last walk never travel to the host): k_rebuild_decide writes
 // Control::rebuild_flag, and bonsai_block_tick enqueues the build chain behind Gate{rebuild_flag, 1} and the refresh
 // behind Gate{rebuild_flag, 0} (internal.cuh); the side not taken costs its empty launches.
@@ -15,7 +19,7 @@ namespace bonsai {
 
 __global__ void k_rebuild_decide(Control* __restrict__ ctl, float factor) {
     const bool have_ref = ctl->tree_fresh == 0u;
-    const bool rebuild = have_ref && ctl->ipp_last > __dmul_rn((double)factor, ctl->ipp_ref);
+    const bool rebuild = ctl->status != 0 || (have_ref && ctl->ipp_last > __dmul_rn((double)factor, ctl->ipp_ref));
     ctl->rebuild_flag = rebuild ? 1u : 0u;
     ctl->n_decisions += 1u;
     if (rebuild) ctl->n_rebuilds += 1u;

@@ -804,13 +804,14 @@ cudaError_t stage_reorder(Ctx* c, bool write_keys) {
 // After the reorder of a fresh sort: put the runs of equal leading key bits in order of their remaining bits -- short
 // runs in place, long ones (coincident particles, clumps far smaller than the cells the passes resolve) by
 // k_sort_long_runs, which returns at once when there are none.  Scratch of the long-run sort: the pair buffers and the
-// load-order key words (dead after the passes) and the fp64 moment array (not yet written).
+// load-order key words (dead after the passes) and tie_pos, an n-sized array of its own (the cell arrays are sized by
+// cap_cells, which the caller may set far below n).
 cudaError_t stage_sort_ties(Ctx* c) {
     Buffers& b = c->b;
     const uint32_t cut = (uint32_t)(kRadixBits * sort_first_pass(c));  // low bits of the mid word the passes skipped
     k_sort_ties<<<div_up(div_up(c->n, 4), 256), 256, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
                                                           b.ctl, b.long_start, cut, c->gate);
-    LongRunScratch sc{b.pair_key[0], b.idx[1], b.key[0][0], b.key[0][1], b.key[0][2], reinterpret_cast<float4*>(b.c_mom)};
+    LongRunScratch sc{b.pair_key[0], b.idx[1], b.key[0][0], b.key[0][1], b.key[0][2], b.tie_pos};
     k_sort_long_runs<<<c->num_sms, kLongWarps * 32, 0, c->stream>>>(b.key[1][0], b.key[1][1], b.key[1][2], c->perm, b.sorted_pos, c->n,
                                                                  b.ctl, b.long_start, sc, cut, c->gate);
     c->launches += 2;

@@ -149,6 +149,39 @@ def test_device_side_rebuild_decision_follows_the_oracle_policy():
            ipp_ref=float(pol.ref), ipp_last=float(pol.last))
 
 
+def test_auto_ticks_recover_from_a_capacity_overflow():
+    """bonsai.h: a build clears the sticky status.  With rebuild = -1 the library must therefore rebuild on the tick
+    after an overflow (a refreshed tick would find the status set, and multipoles and walk return at once on it):
+    the tick after the overflow has to give what a fresh context gives for the same state with rebuild = 1."""
+    n, theta, eps, eta, dt_max, kmax = 5000, 0.75, 0.01, 0.3, 1 / 64, 2
+    pm, vel = W.plummer(n, with_velocities=True)
+    small = pm.copy()
+    small[1000:, :3] = np.float32(np.abs(pm[:, :3]).max() * 1.5)     # 4000 coincident particles: ~270 cells
+    assert O.build(small).tree.n_cells < 700 < O.build(pm).tree.n_cells
+    b = Bonsai(n, cap_cells=700)
+    p_d, v_d = _dev(pm), _dev(O._vel4(vel))
+    a_d = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+    r_d = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    b.block_tick(p_d, v_d, a_d, r_d, 0, theta, eps, eta, dt_max, kmax, rebuild=True)   # ~1200 cells: overflow
+    with pytest.raises(BonsaiError) as e:
+        b.sync()
+    assert e.value.code == -3
+    # the caller repairs its state in the same arrays (the context still "has a tree" for them) and lets the device decide
+    p_d.copy_(_dev(small)); v_d.zero_(); a_d.zero_(); r_d.zero_()
+    fresh = Bonsai(n)
+    p2, v2, a2, r2 = p_d.clone(), v_d.clone(), a_d.clone(), r_d.clone()
+    for tick in (3, 4, 5):                     # tick 3 walks every particle (all on rung 0), 4 and 5 the deeper rungs
+        b.block_tick(p_d, v_d, a_d, r_d, tick, theta, eps, eta, dt_max, kmax, rebuild=-1)
+        b.sync()                                                                      # status cleared by the rebuild
+        fresh.block_tick(p2, v2, a2, r2, tick, theta, eps, eta, dt_max, kmax, rebuild=(tick == 3))
+        fresh.sync()
+        if tick == 3:
+            assert b.rebuild_stats()["n_rebuilds"] == 1
+        for x, y in ((p_d, p2), (v_d, v2), (a_d, a2), (r_d, r2)):
+            assert torch.equal(x, y), tick
+        assert float(a_d[:, :3].abs().max()) > 0
+
+
 def test_block_tick_errors():
     n = 1000
     pm, vel = W.plummer(n, with_velocities=True)

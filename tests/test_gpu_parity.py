@@ -497,6 +497,42 @@ def test_graph_replay_is_bit_identical_to_the_staged_calls():
     assert b.stage_ms()["walk"] > 0
 
 
+def test_stage_times_survive_more_runs_than_event_pairs():
+    """bonsai_get_stage_ms sums a stage over ALL its executions since the last call: a stage that runs more often than it
+    has event pairs (8) folds the finished intervals into a host-side sum instead of overwriting them."""
+    n = 20_000
+    b = Bonsai(n)
+    d_pm = _dev(W.plummer(n))
+    b.step(d_pm, 0.75, 0.01); b.sync()
+    b.set_timing(True)
+    b.step(d_pm, 0.75, 0.01)
+    one = b.stage_ms()
+    for _ in range(21):
+        b.step(d_pm, 0.75, 0.01)
+    many = b.stage_ms()
+    for k in ("sort", "build", "multipoles", "walk"):
+        assert one[k] > 0 and many[k] > 14 * one[k], (k, one[k], many[k])    # 8 re-used pairs would give <= ~8x
+    assert sum(b.stage_ms().values()) == 0.0                                  # read and reset
+
+
+def test_graph_capture_pauses_and_comes_back():
+    """A caller that hands over a new output buffer on every call makes every call a graph miss: after 16 in a row the
+    library stops capturing -- for 256 calls, not for good.  Once the caller's buffers repeat again, replays resume."""
+    n = 2000
+    b = Bonsai(n)
+    d_pm = _dev(W.plummer(n))
+    ref = b.step(d_pm, 0.75, 0.01).clone()
+    outs = [torch.empty((n, 4), dtype=torch.float32, device="cuda") for _ in range(40)]
+    for o in outs:                                             # 40 distinct keys: misses, then the pause
+        assert torch.equal(b.step(d_pm, 0.75, 0.01, None, o), ref)
+    r0 = b.graph_replays()
+    fixed = outs[-1]
+    for _ in range(300):                                       # runs through the rest of the pause, then captures again
+        b.step(d_pm, 0.75, 0.01, None, fixed)
+    assert torch.equal(fixed, ref)
+    assert b.graph_replays() > r0 + 10
+
+
 def test_team_walks_are_deterministic():
     """Team walks (several warps per group over a shared stack, partial sums folded in member order) give bit-identical
     results and counts from run to run, for the 8-warp and the 16-warp team kernel."""
@@ -531,6 +567,28 @@ def test_status_is_cleared_by_the_next_build():
         b.sync()
         check_structure(b, ref)
         check_walk(b, out, ref, count_frac=0.99, eps=0.01, pm=pm)
+
+
+def test_long_tie_run_with_few_cells():
+    """The long-run tie sort (k_sort_long_runs) permutes a run through an n-sized scratch.  That scratch must not be
+    one of the cell arrays: cap_cells is the caller's to choose and may be far below n / 5.  Here 4000 of 5000
+    particles coincide at the corner that sorts last (one run over sorted positions 1000..4999) and cap_cells = 700
+    holds the ~330 cells of the tree; the step must agree with the oracle and repeat bit for bit."""
+    n = 5000
+    pm = W.plummer(n, seed=21)
+    pm[1000:, :3] = np.float32(np.abs(pm[:, :3]).max() * 1.5)   # beyond every other particle on all three axes
+    ref = O.full_step(pm, 0.75, 0.01)
+    assert ref.tree.n_cells < 700 and 5 * 700 < n
+    b = Bonsai(n, cap_cells=700)
+    d_pm = _dev(pm)
+    out = b.step(d_pm, 0.75, 0.01).cpu().numpy()
+    b.sync()
+    check_structure(b, ref)
+    check_groups(b, ref)
+    check_walk(b, out, ref, eps=0.01, pm=pm)
+    again = b.step(d_pm, 0.75, 0.01).cpu().numpy()
+    b.sync()
+    assert np.array_equal(out.view(np.uint32), again.view(np.uint32))
 
 
 def test_two_contexts_from_two_host_threads():
