@@ -469,7 +469,7 @@ def main():
     ap.add_argument("--workload", default="plummer_4m")
     ap.add_argument("--ncrit", type=int, default=64)
     ap.add_argument("--group-mode", dest="group_mode", type=int, default=2)
-    ap.add_argument("--group-cell", dest="group_cell", type=int, default=1024)
+    ap.add_argument("--group-cell", dest="group_cell", type=int, default=512)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -58,7 +58,7 @@ typedef struct {
                             cells with <= group_cell particles [2] (R13).  NOTE: because 0 is a legal value,
                             group_mode is only defaulted when params == NULL.                                 */
     uint32_t cap_cells;  /* [2 n_max + 256] capacity of the cell arrays                                      */
-    uint32_t group_cell; /* [1024] mode 2: a group never crosses the boundary of a cell holding more than
+    uint32_t group_cell; /* [512]  mode 2: a group never crosses the boundary of a cell holding more than
                             group_cell particles (the containers are the cells with count <= group_cell whose
                             parent has more); >= ncrit                                                        */
     uint32_t mac_mode;   /* [0] size and centre of a cell in the opening test ("MAC"): 0 = geometric cell
@@ -346,12 +346,6 @@ uint64_t bonsai_get_graph_replays(bonsai_ctx* ctx);
  * best of three timed launches on `cuda_stream` (CUDA events).  Writes TFLOP/s (FMA = 2 flop) to *tflops_out.
  * Blocks until done.  bench.py reports the walk's flop/s against this next to the derived peak.  EINVAL / ECUDA. */
 int bonsai_measure_fp32_peak(void* cuda_stream, int packed, int iters, double* tflops_out);
-
-/* Measurement support: issue cost of other instruction classes next to packed FMAs.  Every round of a warp is
- * eight FFMA2 plus: kind 0 nothing, 1 eight LOP3 (integer ALU), 2 four LDS.128, 3 two MUFU.RSQ.  Writes the scheduler
- * cycles one round costs (at the device's nominal clock; 16 with nothing added, since an FFMA2 holds the FP32 pipe
- * for two cycles).  What exceeds 16 is what the added instructions cost the walk's interaction loops. */
-int bonsai_measure_issue_mix(void* cuda_stream, int kind, int iters, double* cycles_per_round_out);
 
 const char* bonsai_strerror(int code);
 

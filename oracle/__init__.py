@@ -117,7 +117,7 @@ class Groups:
     bmax: np.ndarray
 
 
-def groups(mode, ncrit, sorted_pos_mass, t: Tree, active_sorted=None, group_cell=1024):
+def groups(mode, ncrit, sorted_pos_mass, t: Tree, active_sorted=None, group_cell=512):
     spm = _f32(sorted_pos_mass)
     n = spm.shape[0]
     act = None if active_sorted is None else np.ascontiguousarray(active_sorted, dtype=np.uint8)
@@ -282,7 +282,7 @@ def tight_mac(sorted_pos_mass, t: Tree):
     return box
 
 
-def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cells=None, group_cell=1024,
+def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cells=None, group_cell=512,
           mac_mode=0) -> Step:
     """O1..O6: box, keys, sort, reorder, tree, groups, multipoles.  active_mask is in LOAD order.
     mac_mode = 1: the tight MAC of R28 (cell size and centre from the particle box)."""
@@ -301,7 +301,7 @@ def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cell
 
 
 def full_step(pos_mass, theta, eps, nleaf=16, ncrit=64, group_mode=2, active_mask=None, sel=None,
-              group_cell=1024, mac_mode=0, order=2) -> Step:
+              group_cell=512, mac_mode=0, order=2) -> Step:
     s = build(pos_mass, nleaf, ncrit, group_mode, active_mask, None, group_cell, mac_mode)
     s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, order)
     return s
@@ -373,7 +373,7 @@ def leapfrog(pos_mass, vel, theta, eps, dt, n_steps, acc_pot=None, **kw):
 
 # ---- row f1: refreshed tree (oracle/refresh_oracle.cpp, R25) --------------------------------
 
-def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, group_cell=1024,
+def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, group_cell=512,
             mac_mode=0) -> Step:
     """The structures of ``prev`` (permutation, keys, cells, group membership) carried over to moved particles.
 

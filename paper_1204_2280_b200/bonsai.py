@@ -32,7 +32,7 @@ SYMBOLS = (
     "bonsai_kick", "bonsai_drift", "bonsai_leapfrog_step", "bonsai_diagnostics", "bonsai_refresh_tree",
     "bonsai_timestep_rungs", "bonsai_active_mask", "bonsai_kick_rungs", "bonsai_block_tick",
     "bonsai_measure_fp32_peak", "bonsai_get_rebuild_stats", "bonsai_step", "bonsai_get_graph_replays",
-    "bonsai_measure_issue_mix", "bonsai_diagnostics_static",
+    "bonsai_diagnostics_static",
 )
 
 
@@ -108,7 +108,6 @@ def lib() -> C.CDLL:
     L.bonsai_diagnostics.argtypes = [vp, vp, vp, vp, u32, vp]
     L.bonsai_diagnostics_static.argtypes = [vp, vp, vp, u32, vp, vp]
     L.bonsai_get_rebuild_stats.argtypes = [vp, C.POINTER(u32), C.POINTER(u32), C.POINTER(C.c_double), C.POINTER(C.c_double)]
-    L.bonsai_measure_issue_mix.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
     L.bonsai_measure_fp32_peak.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
     L.bonsai_strerror.argtypes = [C.c_int]
     L.bonsai_strerror.restype = C.c_char_p
@@ -168,19 +167,6 @@ def diagnostics_static(pos_mass: torch.Tensor, vel: torch.Tensor, acc_pot: torch
         _check(lib().bonsai_diagnostics_static(C.c_void_p(pos_mass.data_ptr()), C.c_void_p(vel.data_ptr()),
                                                C.c_void_p(acc_pot.data_ptr()), n, C.c_void_p(out.data_ptr()), st),
                "bonsai_diagnostics_static")
-    return out
-
-
-def measure_issue_mix(iters: int = 20000) -> dict:
-    """bonsai_measure_issue_mix for the four kinds: scheduler cycles per round of 8 FFMA2 (+ other instructions)."""
-    if not torch.cuda.is_available():
-        raise RuntimeError("libbonsai needs a CUDA device (sm_100a); there is no CPU fallback")
-    out = {}
-    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
-    for kind, name in enumerate(("ffma2_x8", "ffma2_x8+lop3_x8", "ffma2_x8+lds128_x4", "ffma2_x8+mufu_x2")):
-        v = C.c_double(0.0)
-        _check(lib().bonsai_measure_issue_mix(st, kind, int(iters), C.byref(v)), "bonsai_measure_issue_mix")
-        out[name] = float(v.value)
     return out
 
 

@@ -44,7 +44,7 @@ bool resolve_params(uint32_t n_max, const bonsai_params* in, bonsai_params* out)
         p.cap_cells = in->cap_cells;
         p.group_cell = in->group_cell;
     }
-    if (p.group_cell == 0) p.group_cell = 1024;
+    if (p.group_cell == 0) p.group_cell = 512;  // measured at 2^22: 9.75 ms per step against 9.88 (1024) and 10.07 (256)
     if (p.group_cell < p.ncrit) p.group_cell = p.ncrit;
     if (p.cap_cells == 0) {
         unsigned long long cap = 2ull * n_max + 256ull;

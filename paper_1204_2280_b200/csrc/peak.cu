@@ -49,91 +49,7 @@ __global__ void __launch_bounds__(kPeakThreads) k_peak_ffma(int iters, float see
     if (s == 123.456f) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
-// Issue-slot probe: every round is eight packed FMAs (eight independent chains) plus a few instructions of another
-// class placed between them -- does the other class cost issue cycles next to FFMA2, which holds the FP32 pipe for two
-// cycles?  kind 0: nothing; 1: 8 LOP3 (integer ALU pipe); 2: 4 LDS.128 (shared memory, broadcast); 3: 2 MUFU.RSQ.
-template <int KIND>
-__global__ void __launch_bounds__(kPeakThreads) k_issue_mix(int iters, float seed, float* __restrict__ sink) {
-    __shared__ float4 s_src[64];
-    unsigned long long acc[kPeakChains];
-    unsigned long long a, b;
-    const float x = seed + (float)threadIdx.x * 1e-9f;
-    if (threadIdx.x < 64) s_src[threadIdx.x] = make_float4(x, x, x, x);
-    __syncthreads();
-    asm("mov.b64 %0, {%1, %2};" : "=l"(a) : "f"(1.0f - 1e-7f), "f"(1.0f - 2e-7f));
-    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(x), "f"(-x));
-#pragma unroll
-    for (int k = 0; k < kPeakChains; ++k) asm("mov.b64 %0, {%1, %2};" : "=l"(acc[k]) : "f"(x + k), "f"(x - k));
-    uint32_t u[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) u[k] = threadIdx.x * 2654435761u + k;
-    float4 q[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) q[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-    float r0 = 1.0f + x, r1 = 2.0f + x;
-    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(s_src);
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int k = 0; k < kPeakChains; ++k) {
-            asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(acc[k]) : "l"(acc[k]), "l"(a), "l"(b));
-            if (KIND == 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[k]) : "r"(u[(k + 1) & 7]), "r"(i));
-            if (KIND == 2 && (k & 1))
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                             : "=f"(q[k >> 1].x), "=f"(q[k >> 1].y), "=f"(q[k >> 1].z), "=f"(q[k >> 1].w)
-                             : "r"(sa + 16u * (uint32_t)k));  // fixed addresses: no integer work rides along
-            if (KIND == 3 && k == 1) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(r0));
-            if (KIND == 3 && k == 5) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(r1));
-        }
-    }
-    float s = r0 + r1;
-#pragma unroll
-    for (int k = 0; k < kPeakChains; ++k) {
-        float lo, hi;
-        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(acc[k]));
-        s += lo + hi + (float)u[k];
-    }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) s += q[k].x + q[k].y + q[k].z + q[k].w;
-    if (s == 123.456f) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
 }  // namespace bonsai
-
-using namespace bonsai;
-
-extern "C" int bonsai_measure_issue_mix(void* cuda_stream, int kind, int iters, double* cycles_per_round_out) {
-    if (!cycles_per_round_out || iters < 1 || kind < 0 || kind > 3) return BONSAI_EINVAL;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    int dev = 0, sms = 0, khz = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev) != cudaSuccess)
-        return BONSAI_ECUDA;
-    const int blocks = sms * 8;
-    cudaEvent_t e0, e1;
-    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return BONSAI_ECUDA;
-    float best = 0.0f;
-    for (int rep = 0; rep < 4; ++rep) {
-        cudaEventRecord(e0, st);
-        switch (kind) {
-            case 0: k_issue_mix<0><<<blocks, kPeakThreads, 0, st>>>(iters, 0.5f, nullptr); break;
-            case 1: k_issue_mix<1><<<blocks, kPeakThreads, 0, st>>>(iters, 0.5f, nullptr); break;
-            case 2: k_issue_mix<2><<<blocks, kPeakThreads, 0, st>>>(iters, 0.5f, nullptr); break;
-            default: k_issue_mix<3><<<blocks, kPeakThreads, 0, st>>>(iters, 0.5f, nullptr); break;
-        }
-        cudaEventRecord(e1, st);
-        if (cudaEventSynchronize(e1) != cudaSuccess) return BONSAI_ECUDA;
-        float ms = 0.0f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        if (rep > 0 && (best == 0.0f || ms < best)) best = ms;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    if (cudaGetLastError() != cudaSuccess || best <= 0.0f) return BONSAI_ECUDA;
-    // 64 warps per SM = 16 per scheduler: cycles one scheduler spends per round of one warp, at the nominal clock
-    const double rounds_per_scheduler = 16.0 * (double)iters;
-    *cycles_per_round_out = (double)best * 1e-3 * (double)khz * 1e3 / rounds_per_scheduler;
-    return BONSAI_OK;
-}
 
 using namespace bonsai;
 

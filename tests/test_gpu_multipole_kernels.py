@@ -60,7 +60,7 @@ def test_tiles_kernel_repeated_steps_of_different_sizes():
         out = b.step(_dev(pm), 0.75, 0.01).cpu().numpy()
         b.sync()
         check_structure(b, ref)
-        check_walk(b, out, ref, count_frac=0.99, eps=0.01, pm=pm)
+        check_walk(b, out, ref, count_frac=0.99 if n < 5000 else 0.999, eps=0.01, pm=pm)
 
 
 def test_tiles_kernel_on_a_refreshed_tree_and_with_the_tight_mac():

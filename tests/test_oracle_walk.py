@@ -112,6 +112,12 @@ def test_lists_account_for_all_mass_exactly_once(mode, ncrit, theta):
     for G in range(0, g.n_groups, max(1, g.n_groups // 40)):
         mem = g.active_list[g.first[G]:g.first[G] + g.count[G]]
         assert len(set(w.n_pc[mem])) == 1 and len(set(w.n_pp[mem])) == 1
+        # oracle_walk carries its own copy of the traversal: it must visit exactly the lists oracle_walk_lists returns
+        # (the copy the mass-accounting and stated-inequality pins run on), group by group (R21: n_pc = accepted cells,
+        # n_pp = particles of the opened leaves minus the sink itself)
+        pc, pp = O.walk_lists(theta, t, g.bmin[G], g.bmax[G])
+        assert int(w.n_pc[mem[0]]) == len(pc)
+        assert int(w.n_pp[mem[0]]) + 1 == int(t.count[pp].astype(np.int64).sum())
 
 
 def test_mac_is_the_stated_inequality():
