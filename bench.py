@@ -59,7 +59,8 @@ def oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, walk_budge
     All stages before the walk run in full; the walk (>= 98 % of the oracle's time) is first probed on 64
     groups, then timed on every `stride`-th group with `stride` the smallest power of two that keeps it within
     `walk_budget_s`, and scaled by n_particles / n_sinks_sampled (the groups are evenly spaced along the Morton curve).
-    Returns (estimated seconds of one full step, description of the sample).
+    Returns (estimated seconds of one full step, description of the sample, {"stride", "measured_s"}): the third
+    value says what was actually executed -- every `stride`-th group, `measured_s` seconds of wall clock.
     """
     import oracle as O
     t0 = time.perf_counter()
@@ -81,11 +82,11 @@ def oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, walk_budge
     est = t_build + t_walk * (s.groups.n_active / n_sinks)
     what = (f"all pre-walk stages on all {pm.shape[0]} particles ({t_build:.2f} s) + walk of {len(sel)} of {ng} "
             f"groups (every {stride}th, {n_sinks} sinks, {t_walk:.2f} s) scaled by {s.groups.n_active}/{n_sinks}")
-    return est, what
+    return est, what, {"stride": int(stride), "measured_s": float(t_build + t_walk)}
 
 
 def cpu_baseline(pm, theta, eps, ncrit, group_mode, group_cell, budget_s=12.0):
-    est, what = oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, budget_s)
+    est, what, _ = oracle_step_sample(pm, theta, eps, ncrit, group_mode, group_cell, budget_s)
     return {"value": pm.shape[0] / est, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
             "est_full_step_s": est}
 
@@ -130,10 +131,11 @@ def run_reference(args):
     # within two minutes
     for _ in range(min(args.warmup, 1)):
         oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 2.0)
-    ests, what = [], ""
+    ests, measured, what, info = [], [], "", {"stride": 1}
     for _ in range(args.steps):
-        est, what = oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 4.0)
+        est, what, info = oracle_step_sample(pm, theta, eps, args.ncrit, args.group_mode, args.group_cell, 4.0)
         ests.append(est)
+        measured.append(info["measured_s"])
     est = float(np.mean(ests))
     value = n / est
     line = {
@@ -145,6 +147,9 @@ def run_reference(args):
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
+        # ms_per_step is an EXTRAPOLATION: each of the `steps` executed every stride-th group's walk (plus all pre-walk
+        # stages) in measured_s_per_step seconds of wall clock and scaled it to all sinks
+        "sampled": info["stride"] > 1, "stride": info["stride"], "measured_s_per_step": float(np.mean(measured)),
     }
     print(json.dumps(line), flush=True)
     return 0
