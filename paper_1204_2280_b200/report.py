@@ -116,6 +116,53 @@ def block_step(reps: int) -> dict:
     return res
 
 
+def block_ticks(reps: int) -> dict:
+    """bonsai_block_tick end to end (R26, R27, R30): ms per tick over one full cycle of
+    2^kmax ticks at N = 2^20 with the tree rebuilt every tick, refreshed every tick, or rebuilt when the device says so,
+    next to the all-active tick (kmax = 0) -- the tick-time reduction to hold against N / N_active."""
+    del reps
+    cfg = W.CONFIGS["plummer_1m"]
+    n, eps, theta = cfg["n"], cfg["eps"], cfg["theta"]
+    eta, dt_max, kmax = 0.3, 1.0 / 32, 4      # rungs 0 (halo) .. 4 (core) all populated on the Plummer sphere
+    pm_h, vel_h = W.plummer(n, with_velocities=True)
+    v4 = np.zeros((n, 4), np.float32)
+    v4[:, :3] = vel_h
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    res = {"n": n, "theta": theta, "eta": eta, "dt_max": dt_max, "kmax": kmax, "modes": {}}
+    for label, rebuild in (("all_active_kmax0", 1), ("rebuild", 1), ("refresh", 0), ("device_decides", -1)):
+        pm, vel = torch.from_numpy(pm_h).cuda(), torch.from_numpy(v4).cuda()
+        b = Bonsai(n)
+        acc = b.step(pm, theta, eps).clone()
+        km = 0 if label == "all_active_kmax0" else kmax
+        rung = b.timestep_rungs(acc, eta, eps, dt_max, km)
+        cycle = 1 << km
+        n_ticks = 2 * cycle if km else 8
+        rows = []
+        for tick in range(n_ticks):                      # the first cycle is warm-up (and gives `refresh` its tree)
+            n_act = int(b.active_mask(rung, km, tick + 1).sum())         # a host read, outside the event pair
+            rb = 1 if (tick == 0 and rebuild == 0) else rebuild
+            e0.record()
+            b.block_tick(pm, vel, acc, rung, tick, theta, eps, eta, dt_max, km, rebuild=rb)
+            e1.record()
+            e1.synchronize()
+            if tick >= n_ticks // 2:
+                rows.append((e0.elapsed_time(e1), n_act))
+        ms = [r[0] for r in rows]
+        act = [r[1] for r in rows]
+        res["modes"][label] = {"ticks_timed": len(rows), "ms_per_tick_mean": float(np.mean(ms)), "ms_per_tick_min": float(min(ms)),
+                               "ms_per_tick_max": float(max(ms)), "ticks_per_s": 1e3 * len(ms) / float(sum(ms)),
+                               "n_active_mean": float(np.mean(act)), "n_over_n_active": n / max(float(np.mean(act)), 1.0),
+                               "ms_by_tick": [round(x, 4) for x in ms], "n_active_by_tick": act}
+        if rebuild < 0:
+            res["modes"][label]["rebuild_stats"] = b.rebuild_stats()
+        b.sync()
+        del b
+    full = res["modes"]["all_active_kmax0"]["ms_per_tick_mean"]
+    for label, d in res["modes"].items():
+        d["tick_time_reduction"] = full / d["ms_per_tick_mean"]
+    return res
+
+
 def scaling(reps: int) -> dict:
     rows = {}
     beyond = {"plummer_16m": dict(n=1 << 24, eps=0.0008, theta=0.75)}  # four times the paper's largest N (working set 4x L2)
@@ -329,13 +376,21 @@ def markdown(doc: dict) -> str:
             o += [f"| {name} | {th} | {r['acc_err_median']:.2e} | {r['acc_err_p99']:.2e} | {r['pp_per_particle']:.0f} | "
                   f"{r['pc_per_particle']:.0f} | {r['walk_ms']:.3f} |" for th, r in by.items()]
         o.append("")
+    if "block_ticks" in doc:
+        d = doc["block_ticks"]
+        o += [f"## bonsai_block_tick end to end, N = {d['n']}, kmax = {d['kmax']} (one cycle of {1 << d['kmax']} ticks, after one warm-up cycle)\n",
+              "| tree per tick | ms per tick (mean) | min | max | ticks/s | mean N_active | N / N_active | tick-time reduction vs all-active |",
+              "|---|---|---|---|---|---|---|---|"]
+        o += [f"| {k} | {r['ms_per_tick_mean']:.3f} | {r['ms_per_tick_min']:.3f} | {r['ms_per_tick_max']:.3f} | {r['ticks_per_s']:.0f} | "
+              f"{r['n_active_mean']:.0f} | {r['n_over_n_active']:.1f} | {r['tick_time_reduction']:.2f} |" for k, r in d["modes"].items()]
+        o.append("")
     return "\n".join(o)
 
 
 def main() -> None:
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--reps", type=int, default=5)
-    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "scaling", "merger", "mac"), default=None)
+    ap.add_argument("--only", choices=("theta_sweep", "leapfrog", "block_step", "block_ticks", "scaling", "merger", "mac"), default=None)
     ap.add_argument("--markdown", default=None, help="also write the tables as markdown to this file")
     ap.add_argument("--from-json", dest="from_json", default=None,
                     help="render --markdown from an earlier JSON output instead of measuring (needs no GPU)")
@@ -353,7 +408,8 @@ def main() -> None:
         return
     if not torch.cuda.is_available():
         raise SystemExit("report: no CUDA device -- libbonsai has no CPU fallback")
-    parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "scaling": scaling,
+    parts = {"theta_sweep": theta_sweep, "leapfrog": leapfrog, "block_step": block_step, "block_ticks": block_ticks,
+             "scaling": scaling,
              "merger": merger, "mac": mac_variants}
     doc = {k: f(args.reps) for k, f in parts.items() if args.only in (None, k)}
     print(json.dumps(doc, indent=1))
