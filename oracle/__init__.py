@@ -300,10 +300,18 @@ def build(pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=None, cap_cell
     return Step(lo, side, k, perm, spm, sk, t, g)
 
 
+def _walk_maybe_threaded(theta, eps, s: "Step", sel, order, threads):
+    """walk(), or the same oracle_walk fanned out over host threads (walk_threads: no arithmetic of its own)."""
+    if threads <= 1:
+        return walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, order)
+    sel = np.arange(s.groups.n_groups, dtype=np.uint32) if sel is None else sel
+    return walk_threads(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, threads, order)
+
+
 def full_step(pos_mass, theta, eps, nleaf=16, ncrit=64, group_mode=2, active_mask=None, sel=None,
-              group_cell=512, mac_mode=0, order=2) -> Step:
+              group_cell=512, mac_mode=0, order=2, threads=1) -> Step:
     s = build(pos_mass, nleaf, ncrit, group_mode, active_mask, None, group_cell, mac_mode)
-    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, order)
+    s.walk = _walk_maybe_threaded(theta, eps, s, sel, order, threads)
     return s
 
 
@@ -398,9 +406,9 @@ def refresh(prev: Step, pos_mass, nleaf=16, ncrit=64, group_mode=2, active_mask=
     return Step(prev.lo, prev.side, prev.keys, prev.perm, spm, prev.sorted_keys, t, g)
 
 
-def refreshed_step(prev: Step, pos_mass, theta, eps, sel=None, order=2, **kw) -> Step:
+def refreshed_step(prev: Step, pos_mass, theta, eps, sel=None, order=2, threads=1, **kw) -> Step:
     s = refresh(prev, pos_mass, **kw)
-    s.walk = walk(theta, eps, s.sorted_pos_mass, s.tree, s.groups, sel, order)
+    s.walk = _walk_maybe_threaded(theta, eps, s, sel, order, threads)
     return s
 
 
@@ -475,6 +483,7 @@ def block_tick(pm, v4, ap, rung, tick, theta, eps, eta, dt_max, kmax, prev: Step
     """One tick of the block scheme (R27), in place on pm / v4 / ap / rung.  prev: refresh this Step's tree instead
     of rebuilding (R25).  policy: decide between the two with R30 (prev must then be the last tick's Step, or None
     when no tree exists yet).  Returns (the Step of this tick, number of active particles walked)."""
+    threads = kw.pop("threads", 1)          # host threads of the walk (fan-out only)
     m0 = active_at(rung, kmax, tick)
     kick_rungs(v4, ap, rung, m0, dt_max)
     drift(pm, v4, np.float32(np.ldexp(np.float32(dt_max), -kmax)))
@@ -482,11 +491,11 @@ def block_tick(pm, v4, ap, rung, tick, theta, eps, eta, dt_max, kmax, prev: Step
     if policy is not None and prev is not None and policy.decide():
         prev = None
     if prev is None:
-        s = full_step(pm, theta, eps, active_mask=m1, **kw)
+        s = full_step(pm, theta, eps, active_mask=m1, threads=threads, **kw)
         if policy is not None:
             policy.built()
     else:
-        s = refreshed_step(prev, pm, theta, eps, active_mask=m1, **kw)
+        s = refreshed_step(prev, pm, theta, eps, active_mask=m1, threads=threads, **kw)
     if policy is not None:
         policy.record(s.walk, m1[s.perm].astype(bool))
     sel = m1[s.perm].astype(bool)

@@ -182,6 +182,60 @@ def test_auto_ticks_recover_from_a_capacity_overflow():
         assert float(a_d[:, :3].abs().max()) > 0
 
 
+def test_block_ticks_at_config2_size_follow_the_oracle_tick_by_tick():
+    """One rebuilt and one refreshed bonsai_block_tick at N = 2^20 (BASELINE configs[2] / [4] size: tiled multipole
+    kernel, plain and team walk kernels, 4-pass sort), each against oracle.block_tick started from the state the GPU
+    had before the tick (stage isolation): opening kick + drift are single fp32 FMAs on identical inputs
+    -> positions bit-exact, hence the same permutation and tree; the walked particles' counts identical for >= 99.9 %,
+    acc / pot within 1e-4 max / 1e-6 median; rows of particles that were not walked untouched; new rungs equal except
+    where |a| sits on a rung boundary.  The oracle's walk is fanned out over the host's cores (walk_threads)."""
+    import os
+    threads = max(1, min(16, os.cpu_count() or 1))
+    cfg = W.CONFIGS["plummer_1m"]
+    n, theta, eps = cfg["n"], cfg["theta"], cfg["eps"]
+    eta, dt_max, kmax = 0.3, 1 / 32, 2
+    pm, vel = W.plummer(n, with_velocities=True)
+    b = Bonsai(n)
+    p_d, v_d = _dev(pm), _dev(O._vel4(vel))
+    a_d = b.step(p_d, theta, eps).clone()
+    r_d = b.timestep_rungs(a_d, eta, eps, dt_max, kmax)
+    prev = None
+    u = lambda x: np.ascontiguousarray(x).view(np.uint32)
+    for tick, rebuild in ((0, True), (1, False)):
+        p, v, ap, r = (x.cpu().numpy().copy() for x in (p_d, v_d, a_d, r_d))
+        a_before, v_before = ap.copy(), v.copy()
+        m0, m1 = O.active_at(r, kmax, tick).astype(bool), O.active_at(r, kmax, tick + 1).astype(bool)
+        b.block_tick(p_d, v_d, a_d, r_d, tick, theta, eps, eta, dt_max, kmax, rebuild=rebuild)
+        b.sync()
+        s, na = O.block_tick(p, v, ap, r, tick, theta, eps, eta, dt_max, kmax, prev=None if rebuild else prev,
+                             threads=threads)
+        prev = s
+        assert n // 20 < na < n and na == int(m1.sum())
+        pg, vg, ag, rg = (x.cpu().numpy() for x in (p_d, v_d, a_d, r_d))
+        assert np.array_equal(u(pg), u(p))                                 # kick + drift: bit-exact
+        assert np.array_equal(b.perm(), s.perm)                            # same tree (rebuilt or frozen)
+        n_pp, n_pc = b.counts()
+        w = s.walk
+        same = (n_pp[s.perm] == w.n_pp) & (n_pc[s.perm] == w.n_pc)
+        assert same[m1[s.perm]].mean() >= 0.999
+        ea = np.linalg.norm(ag[m1, :3].astype(np.float64) - ap[m1, :3], axis=1) / np.linalg.norm(ap[m1, :3].astype(np.float64), axis=1)
+        ep = np.abs((ag[m1, 3].astype(np.float64) - ap[m1, 3]) / ap[m1, 3])
+        assert ea.max() <= 1e-4 and np.median(ea) <= 1e-6 and ep.max() <= 1e-4, (ea.max(), np.median(ea), ep.max())
+        assert np.array_equal(u(ag[~m1]), u(a_before[~m1]))                # not walked: force row untouched
+        idle = ~m0 & ~m1
+        assert np.array_equal(u(vg[idle]), u(v_before[idle]))              # neither kick touched them
+        only_open = m0 & ~m1
+        assert np.array_equal(u(vg[only_open]), u(v[only_open]))           # opening kick only: bit-exact
+        dv = np.abs(vg[m1, :3].astype(np.float64) - v[m1, :3]).max(axis=1)
+        assert dv.max() <= 2e-4 * np.abs(ap[m1, :3]).max() * dt_max        # closing kick: the force tolerance times dt
+        flips = float((rg != r).mean())
+        assert flips < 1e-3, flips
+        from test_gpu_parity import record
+        record("block tick at 2^20", tick=tick, rebuilt=bool(rebuild), walked=int(na), count_frac=float(same[m1[s.perm]].mean()),
+               n=int(n), n_checked=int(na), n_borderline_mismatch=int((~same[m1[s.perm]]).sum()), acc_max=float(ea.max()),
+               acc_med=float(np.median(ea)), pot_max=float(ep.max()), pot_med=float(np.median(ep)), rung_flips=flips)
+
+
 def test_block_tick_errors():
     n = 1000
     pm, vel = W.plummer(n, with_velocities=True)
